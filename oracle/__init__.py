@@ -1,0 +1,195 @@
+"""ctypes loader for the CPU oracle (oracle/cos_oracle.c).
+
+TEST INFRASTRUCTURE ONLY: imported by tests/, __graft_entry__.smoke() and bench.py's
+cpu_baseline / --impl reference legs.  The product package paper_2501_00675_b200 never imports
+this module and this module never imports the product package.
+
+Every wrapper only marshals numpy arrays into the C functions; the arithmetic is all in
+cos_oracle.c / cos_oracle_core.inc, where each function cites the passage of the paper
+ or the DESIGN.md reading it follows.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SO = os.path.join(_HERE, "liboracle.so")
+_SRC = [os.path.join(_HERE, "cos_oracle.c"), os.path.join(_HERE, "cos_oracle_core.inc")]
+_lib = None
+
+_c_double_p = ctypes.POINTER(ctypes.c_double)
+_c_int_p = ctypes.POINTER(ctypes.c_int)
+
+
+def build(force: bool = False) -> str:
+    """Compile liboracle.so with gcc if it is missing or older than its sources."""
+    stale = force or not os.path.exists(_SO) or any(
+        os.path.getmtime(s) > os.path.getmtime(_SO) for s in _SRC)
+    if stale:
+        cmd = ["gcc", "-O2", "-std=c11", "-ffp-contract=off", "-fopenmp", "-shared", "-fPIC",
+               _SRC[0], "-o", _SO, "-lm"]
+        subprocess.run(cmd, check=True, cwd=_HERE)
+    return _SO
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        build()
+        lib = ctypes.CDLL(_SO)
+        lib.oracle_build_G.restype = None
+        lib.oracle_build_G.argtypes = [ctypes.c_int, ctypes.c_longlong, _c_int_p, _c_double_p,
+                                       _c_double_p, _c_double_p, ctypes.c_int, ctypes.c_int,
+                                       ctypes.c_int, ctypes.c_double, ctypes.c_double,
+                                       _c_double_p, _c_double_p]
+        for name in ("oracle_eval", "oracle_eval_f80"):
+            f = getattr(lib, name)
+            f.restype = ctypes.c_int
+            f.argtypes = [ctypes.c_int, ctypes.c_longlong, _c_double_p, _c_double_p, _c_double_p,
+                          ctypes.c_double, _c_double_p, _c_double_p, ctypes.c_int]
+        lib.oracle_minors.restype = None
+        lib.oracle_minors.argtypes = [ctypes.c_int, _c_double_p, _c_double_p]
+        lib.oracle_DC.restype = None
+        lib.oracle_DC.argtypes = [ctypes.c_int, _c_double_p, _c_double_p, _c_double_p,
+                                  _c_double_p, _c_double_p]
+        lib.oracle_abs_sum.restype = ctypes.c_double
+        lib.oracle_abs_sum.argtypes = [ctypes.c_int, _c_double_p, _c_double_p, _c_double_p, _c_double_p]
+        lib.oracle_abs_sums.restype = None
+        lib.oracle_abs_sums.argtypes = [ctypes.c_int, ctypes.c_longlong, _c_double_p, _c_double_p,
+                                        _c_double_p, ctypes.c_double, _c_double_p, _c_double_p,
+                                        ctypes.c_int]
+        lib.oracle_bruteforce.restype = ctypes.c_int
+        lib.oracle_bruteforce.argtypes = [ctypes.c_int, _c_double_p, _c_double_p, _c_double_p,
+                                          _c_double_p, _c_double_p,
+                                          ctypes.POINTER(ctypes.c_longlong)]
+        lib.oracle_max_threads.restype = ctypes.c_int
+        lib.oracle_max_threads.argtypes = []
+        _lib = lib
+    return _lib
+
+
+def _f64(a):
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+def _p(a):
+    return a.ctypes.data_as(_c_double_p)
+
+
+def max_threads() -> int:
+    return int(_load().oracle_max_threads())
+
+
+def build_G(xy, tau, table_up, table_dn, beta, g_diag=0.0):
+    """G assembly.  xy [B,n,2] int32, tau [B,n]; tables [Lx,Ly,ntau].  Returns (Gup, Gdn) [B,n,n]."""
+    lib = _load()
+    xy = np.ascontiguousarray(xy, dtype=np.int32)
+    tau = _f64(tau)
+    table_up = _f64(table_up)
+    table_dn = table_up if table_dn is None else _f64(table_dn)
+    B, n = tau.shape
+    Lx, Ly, ntau = table_up.shape
+    assert xy.shape == (B, n, 2) and table_dn.shape == table_up.shape
+    Gup = np.empty((B, n, n), dtype=np.float64)
+    Gdn = np.empty((B, n, n), dtype=np.float64)
+    lib.oracle_build_G(n, B, xy.ctypes.data_as(_c_int_p), _p(tau), _p(table_up), _p(table_dn),
+                       Lx, Ly, ntau, float(beta), float(g_diag), _p(Gup), _p(Gdn))
+    return Gup, Gdn
+
+
+def _eval(fname, Gup, Gdn, U, u, threads):
+    lib = _load()
+    Gup = _f64(Gup)
+    Gdn = Gup if Gdn is None else _f64(Gdn)
+    B, n, n2 = Gup.shape
+    assert n == n2 and Gdn.shape == Gup.shape and 1 <= n <= 20
+    up = None
+    if u is not None:
+        u = _f64(u)
+        assert u.shape == (B, n)
+        up = _p(u)
+    out_all = np.empty(B, dtype=np.float64)
+    out_conn = np.empty(B, dtype=np.float64)
+    used = getattr(lib, fname)(n, B, _p(Gup), _p(Gdn), up, float(U), _p(out_all), _p(out_conn),
+                               int(threads))
+    return out_all, out_conn, used
+
+
+def eval_all_connected(Gup, Gdn=None, U=1.0, u=None, threads=0):
+    """Returns (all[B], connected[B]) in FP64.  threads<=0: every OpenMP thread."""
+    a, c, _ = _eval("oracle_eval", Gup, Gdn, U, u, threads)
+    return a, c
+
+
+def eval_all_connected_timed(Gup, Gdn=None, U=1.0, u=None, threads=0):
+    """Like eval_all_connected but also returns the thread count the C code used."""
+    return _eval("oracle_eval", Gup, Gdn, U, u, threads)
+
+
+def eval_all_connected_f80(Gup, Gdn=None, U=1.0, u=None, threads=0):
+    """Long-double accumulators ("truth" for conditioning reports)."""
+    a, c, _ = _eval("oracle_eval_f80", Gup, Gdn, U, u, threads)
+    return a, c
+
+
+def minors(W):
+    """Z[S] = sum over permutations of S of (-1)^cyc prod W, for every subset S.  W [n,n] -> [2^n]."""
+    lib = _load()
+    W = _f64(W)
+    n = W.shape[0]
+    Z = np.empty(1 << n, dtype=np.float64)
+    lib.oracle_minors(n, _p(W), _p(Z))
+    return Z
+
+
+def DC(Gup, Gdn, u):
+    """D[S], C[S] for every subset S of one configuration."""
+    lib = _load()
+    Gup, Gdn, u = _f64(Gup), _f64(Gdn), _f64(u)
+    n = Gup.shape[0]
+    D = np.empty(1 << n, dtype=np.float64)
+    C = np.empty(1 << n, dtype=np.float64)
+    lib.oracle_DC(n, _p(Gup), _p(Gdn), _p(u), _p(D), _p(C))
+    return D, C
+
+
+def abs_sum(Gup, Gdn, u):
+    """Sum of |term| over the connected recursion with every sign dropped (one configuration)."""
+    lib = _load()
+    Gup, Gdn, u = _f64(Gup), _f64(Gdn), _f64(u)
+    return float(lib.oracle_abs_sum(Gup.shape[0], _p(Gup), _p(Gdn), _p(u), None))
+
+
+def abs_sums(Gup, Gdn=None, U=1.0, u=None, threads=0):
+    """Rounding-error scales for a batch: (abs_connected[B], abs_all[B]); see DESIGN.md §3 tolerance."""
+    lib = _load()
+    Gup = _f64(Gup)
+    Gdn = Gup if Gdn is None else _f64(Gdn)
+    B, n, _ = Gup.shape
+    up = None
+    if u is not None:
+        u = _f64(u)
+        up = _p(u)
+    ac = np.empty(B, dtype=np.float64)
+    aa = np.empty(B, dtype=np.float64)
+    lib.oracle_abs_sums(n, B, _p(Gup), _p(Gdn), up, float(U), _p(ac), _p(aa), int(threads))
+    return ac, aa
+
+
+def bruteforce(Gup, Gdn, u):
+    """Plain definition over all (n!)^2 permutation pairs, n <= 8.  Returns (all, connected, count)."""
+    lib = _load()
+    Gup, Gdn, u = _f64(Gup), _f64(Gdn), _f64(u)
+    n = Gup.shape[0]
+    a = ctypes.c_double()
+    c = ctypes.c_double()
+    k = ctypes.c_longlong()
+    rc = lib.oracle_bruteforce(n, _p(Gup), _p(Gdn), _p(u), ctypes.byref(a), ctypes.byref(c),
+                               ctypes.byref(k))
+    if rc != 0:
+        raise ValueError("bruteforce: n out of range")
+    return a.value, c.value, k.value

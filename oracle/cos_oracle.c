@@ -1,0 +1,292 @@
+/*
+ * oracle/cos_oracle.c -- plain, slow, obviously-correct CPU oracle for the CoS hot path of
+ * arxiv/paper_2501_00675 (Sturt & Kozik, "Exploiting Parallelism for Fast Feynman Diagrammatics").
+ *
+ * TEST INFRASTRUCTURE ONLY.  Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+ * --impl reference legs may build, link or call this file.  It shares no code, header, table or
+ * helper with paper_2501_00675_b200/ (the CUDA path) and neither includes the other.
+ *
+ * Contents (each function cites the passage it follows; P:<line> = /root/reference/PAPER.md):
+ *   oracle_build_G          G assembly from a tabulated G0(x,tau)      (BASELINE.json configs; R8, R9, R7)
+ *   oracle_eval / _f80      propagation -> combine -> connected reduction (R1, R5, R6, R10)
+ *   oracle_minors           Z[S] of one species for every subset S     (pinned against LU minors in tests)
+ *   oracle_bruteforce       the plain definition: every pair of permutations, connectivity tested
+ *                           explicitly ("all O(n!) terms", R3)      -- pins oracle_eval for n <= 7
+ *   oracle_abs_sum          conditioning number numerator (R5)
+ *
+ * Pins (tests/test_oracle_*.py, all run without a GPU): brute force n<=5 (and a pure-Python
+ * enumerator written separately), connected-pair counts 1,3,26,426,11064, all = prod(-u) det Gup det Gdn
+ * via numpy.linalg, Z[S] = (-1)^|S| det W[S,S] via numpy.linalg for every S, closed forms at n=1,2,
+ * rank-1 and identity special cases, block-diagonal => 0, relabelling/transpose/diagonal-similarity
+ * invariances, exp/log consistency over set partitions.  No function here is "parity unpinned".
+ *
+ * Build:  gcc -O2 -std=c11 -ffp-contract=off -fopenmp -shared -fPIC cos_oracle.c -o liboracle.so -lm
+ * (-ffp-contract=off: every product and sum below is rounded separately except the one fma() that
+ *  reading R8 writes explicitly.)
+ */
+#include <math.h>
+#include <stddef.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+#define REAL double
+#define FN(name) name##_f64
+#include "cos_oracle_core.inc"
+#undef REAL
+#undef FN
+
+#define REAL long double
+#define FN(name) name##_f80
+#include "cos_oracle_core.inc"
+#undef REAL
+#undef FN
+
+/* ------------------------------------------------------------------------------------------
+ * G assembly (§8(a) a1; BASELINE.json configs: "G0(x,tau) is tabulated ... with 512 tau-points and
+ * linear interpolation; spin-up and spin-down G are n x n FP64").  Readings R7, R8, R9:
+ *   G_s[b][i][j] = G0_s( (x_i - x_j) mod L , tau_i - tau_j )
+ *   table T_s[dx][dy][k] holds G0_s at tau_k = k*beta/(ntau-1), k = 0..ntau-1 (0+ and beta- ends)
+ *   dtau > 0 :  lerp(T, dtau);   dtau <= 0 (i != j): -lerp(T, dtau + beta)   (antiperiodicity)
+ *   lerp: u = dtau*(ntau-1)/beta, k = min(floor(u), ntau-2), value = fma(u-k, T[k+1]-T[k], T[k])
+ *   i == j: g_diag (equal-time diagonal, R7)
+ * xy: [batch][n][2] int32 lattice sites; tau: [batch][n]; Gup,Gdn: [batch][n][n] row-major.
+ * Tup and Tdn may be the same table; Gdn may be NULL (then only Gup is written).
+ */
+static double lerp_table(const double *T, int ntau, double beta, double dtau)
+{
+    const double u = dtau * (double)(ntau - 1) / beta;
+    int k = (int)floor(u);
+    if (k > ntau - 2) k = ntau - 2;
+    if (k < 0) k = 0;
+    return fma(u - (double)k, T[k + 1] - T[k], T[k]);
+}
+
+void oracle_build_G(int n, long long batch, const int *xy, const double *tau,
+                    const double *Tup, const double *Tdn, int Lx, int Ly, int ntau, double beta,
+                    double g_diag, double *Gup, double *Gdn)
+{
+    for (long long b = 0; b < batch; ++b)
+        for (int i = 0; i < n; ++i)
+            for (int j = 0; j < n; ++j) {
+                const size_t o = ((size_t)b * n + i) * n + j;
+                if (i == j) {
+                    Gup[o] = g_diag;
+                    if (Gdn) Gdn[o] = g_diag;
+                    continue;
+                }
+                const int *pi = xy + ((size_t)b * n + i) * 2, *pj = xy + ((size_t)b * n + j) * 2;
+                int dx = (pi[0] - pj[0]) % Lx; if (dx < 0) dx += Lx;
+                int dy = (pi[1] - pj[1]) % Ly; if (dy < 0) dy += Ly;
+                double dtau = tau[(size_t)b * n + i] - tau[(size_t)b * n + j];
+                double sign = 1.0;
+                if (dtau <= 0.0) { dtau += beta; sign = -1.0; }      /* R9: dtau == 0 is 0- */
+                const size_t row = ((size_t)dx * Ly + dy) * (size_t)ntau;
+                Gup[o] = sign * lerp_table(Tup + row, ntau, beta, dtau);
+                if (Gdn) Gdn[o] = sign * lerp_table(Tdn + row, ntau, beta, dtau);
+            }
+}
+
+/* ------------------------------------------------------------------------------------------
+ * Batch evaluation.  Gup,Gdn: [batch][n][n] (may alias); u: NULL or [batch][n]; U used when u NULL.
+ * out_all, out_connected: [batch] (either may be NULL).  threads <= 0: all OpenMP threads.
+ * Returns the number of threads used.
+ */
+int oracle_eval(int n, long long batch, const double *Gup, const double *Gdn,
+                const double *u, double U, double *out_all, double *out_connected, int threads)
+{
+    int used = 1;
+#ifdef _OPENMP
+    if (threads <= 0) threads = omp_get_max_threads();
+    used = threads;
+#pragma omp parallel num_threads(threads)
+#endif
+    {
+        double *work = (double *)malloc(sizeof(double) * work_reals_f64(n));
+        double ubuf[32];
+#ifdef _OPENMP
+#pragma omp for schedule(static)
+#endif
+        for (long long b = 0; b < batch; ++b) {
+            for (int a = 0; a < n; ++a) ubuf[a] = u ? u[(size_t)b * n + a] : U;
+            double all, conn;
+            eval_one_f64(n, Gup + (size_t)b * n * n, Gdn + (size_t)b * n * n, ubuf, work, &all, &conn);
+            if (out_all) out_all[b] = all;
+            if (out_connected) out_connected[b] = conn;
+        }
+        free(work);
+    }
+    return used;
+}
+
+/* Same, every accumulator in long double; results rounded to double on output ("truth" mode). */
+int oracle_eval_f80(int n, long long batch, const double *Gup, const double *Gdn,
+                    const double *u, double U, double *out_all, double *out_connected, int threads)
+{
+    int used = 1;
+#ifdef _OPENMP
+    if (threads <= 0) threads = omp_get_max_threads();
+    used = threads;
+#pragma omp parallel num_threads(threads)
+#endif
+    {
+        long double *work = (long double *)malloc(sizeof(long double) * work_reals_f80(n));
+        double ubuf[32];
+#ifdef _OPENMP
+#pragma omp for schedule(static)
+#endif
+        for (long long b = 0; b < batch; ++b) {
+            for (int a = 0; a < n; ++a) ubuf[a] = u ? u[(size_t)b * n + a] : U;
+            long double all, conn;
+            eval_one_f80(n, Gup + (size_t)b * n * n, Gdn + (size_t)b * n * n, ubuf, work, &all, &conn);
+            if (out_all) out_all[b] = (double)all;
+            if (out_connected) out_connected[b] = (double)conn;
+        }
+        free(work);
+    }
+    return used;
+}
+
+/* Z[S] for every subset S of one n x n matrix W (step 1 alone).  Z: [2^n]. */
+void oracle_minors(int n, const double *W, double *Z)
+{
+    double *A = (double *)malloc(sizeof(double) * ((size_t)n << n));
+    propagate_f64(n, W, -1.0, Z, A);
+    free(A);
+}
+
+/* D[S] and C[S] for every subset of one configuration (steps 1-3), for the exp/log pin. */
+void oracle_DC(int n, const double *Gup, const double *Gdn, const double *u, double *D, double *C)
+{
+    const size_t N = (size_t)1 << n;
+    double *A = (double *)malloc(sizeof(double) * (N * n + 2 * N));
+    double *Zup = A + N * n, *Zdn = Zup + N;
+    propagate_f64(n, Gup, -1.0, Zup, A);
+    propagate_f64(n, Gdn, -1.0, Zdn, A);
+    combine_f64(n, Zup, Zdn, u, D);
+    reduce_connected_f64(n, D, C);
+    free(A);
+}
+
+/* |.|-sum of every term with all signs dropped, one configuration (R5 conditioning numerator). */
+double oracle_abs_sum(int n, const double *Gup, const double *Gdn, const double *u, double *abs_all)
+{
+    long double *work = (long double *)malloc(sizeof(long double) * work_reals_f80(n));
+    long double aa = 0;
+    const long double r = abs_sum_one_f80(n, Gup, Gdn, u, work, &aa);
+    if (abs_all) *abs_all = (double)aa;
+    free(work);
+    return (double)r;
+}
+
+/* Batch form: abs_conn[b], abs_all[b] for every configuration (u NULL -> U).  Error-bound scales:
+ * |fl(connected) - connected| <~ c * eps * abs_conn, |fl(all) - all| <~ c * eps * abs_all. */
+void oracle_abs_sums(int n, long long batch, const double *Gup, const double *Gdn, const double *u,
+                     double U, double *abs_conn, double *abs_all, int threads)
+{
+#ifdef _OPENMP
+    if (threads <= 0) threads = omp_get_max_threads();
+#pragma omp parallel for num_threads(threads) schedule(static)
+#endif
+    for (long long b = 0; b < batch; ++b) {
+        double ubuf[32];
+        for (int a = 0; a < n; ++a) ubuf[a] = u ? u[(size_t)b * n + a] : U;
+        abs_conn[b] = oracle_abs_sum(n, Gup + (size_t)b * n * n, Gdn + (size_t)b * n * n, ubuf, abs_all + b);
+    }
+}
+
+/* ------------------------------------------------------------------------------------------
+ * The plain definition, one configuration, n <= 8 (SURVEY §8(c) "Plain definition"):
+ *   all       = prod_a(-u_a) * sum_{sigma_up, sigma_dn in S_n} (-1)^{cyc(sigma_up)+cyc(sigma_dn)}
+ *                              prod_i Gup[i][sigma_up(i)] * Gdn[i][sigma_dn(i)]
+ *   connected = the same sum restricted to pairs for which the graph on {0..n-1} with edges
+ *               {i, sigma_up(i)} and {i, sigma_dn(i)} is connected
+ *   ("all O(n!) terms"; "-1 ... closing a fermion loop"; R3: (n!)^2 pairs for two species)
+ * n_connected returns the number of connected pairs (must be 1, 3, 26, 426, 11064 for n = 1..5).
+ * Returns 0, or -1 if n is out of range.
+ */
+static int next_permutation_int(int *p, int n)
+{
+    int i = n - 2;
+    while (i >= 0 && p[i] > p[i + 1]) --i;
+    if (i < 0) return 0;
+    int j = n - 1;
+    while (p[j] < p[i]) --j;
+    int t = p[i]; p[i] = p[j]; p[j] = t;
+    for (int a = i + 1, b = n - 1; a < b; ++a, --b) { t = p[a]; p[a] = p[b]; p[b] = t; }
+    return 1;
+}
+
+static int uf_find(int *parent, int x)
+{
+    while (parent[x] != x) x = parent[x];
+    return x;
+}
+
+int oracle_bruteforce(int n, const double *Gup, const double *Gdn, const double *u,
+                      double *out_all, double *out_connected, long long *n_connected)
+{
+    if (n < 1 || n > 8) return -1;
+    int fact = 1;
+    for (int i = 2; i <= n; ++i) fact *= i;
+    int *perm = (int *)malloc(sizeof(int) * (size_t)fact * n);
+    double *tu = (double *)malloc(sizeof(double) * (size_t)fact * 2), *td = tu + fact;
+
+    int p[8];
+    for (int i = 0; i < n; ++i) p[i] = i;
+    int idx = 0;
+    do {                                              /* every permutation, its cycle count, its product */
+        memcpy(perm + (size_t)idx * n, p, sizeof(int) * n);
+        int seen[8] = {0}, cyc = 0;
+        for (int i = 0; i < n; ++i) {
+            if (seen[i]) continue;
+            ++cyc;
+            for (int j = i; !seen[j]; j = p[j]) seen[j] = 1;
+        }
+        double pu = 1.0, pd = 1.0;
+        for (int i = 0; i < n; ++i) { pu *= Gup[i * n + p[i]]; pd *= Gdn[i * n + p[i]]; }
+        const double sg = (cyc & 1) ? -1.0 : 1.0;      /* (-1)^{number of closed fermion loops} */
+        tu[idx] = sg * pu;
+        td[idx] = sg * pd;
+        ++idx;
+    } while (next_permutation_int(p, n));
+
+    double w = 1.0;
+    for (int a = 0; a < n; ++a) w *= -u[a];
+
+    long double sum_all = 0, sum_conn = 0;
+    long long cnt = 0;
+    for (int a = 0; a < fact; ++a)
+        for (int b = 0; b < fact; ++b) {
+            const double term = tu[a] * td[b];
+            sum_all += term;
+            int parent[8];
+            for (int i = 0; i < n; ++i) parent[i] = i;
+            const int *pa = perm + (size_t)a * n, *pb = perm + (size_t)b * n;
+            int comps = n;
+            for (int i = 0; i < n; ++i) {
+                int r0 = uf_find(parent, i), r1 = uf_find(parent, pa[i]);
+                if (r0 != r1) { parent[r0] = r1; --comps; }
+                r0 = uf_find(parent, i); r1 = uf_find(parent, pb[i]);
+                if (r0 != r1) { parent[r0] = r1; --comps; }
+            }
+            if (comps == 1) { sum_conn += term; ++cnt; }
+        }
+    if (out_all) *out_all = (double)((long double)w * sum_all);
+    if (out_connected) *out_connected = (double)((long double)w * sum_conn);
+    if (n_connected) *n_connected = cnt;
+    free(perm);
+    free(tu);
+    return 0;
+}
+
+int oracle_max_threads(void)
+{
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
