@@ -1,0 +1,142 @@
+/*
+ * include/cos.h -- C-ABI boundary of the B200-native CoS evaluation library (libcos_b200.so).
+ *
+ * The library evaluates, for a batch of Monte Carlo vertex configurations, the sum of the integrands
+ * of ALL (cos_eval_all) or all CONNECTED (cos_eval_connected) Feynman diagrams of order n by
+ * combinatorial summation (CoS):  arxiv/paper_2501_00675, Sturt & Kozik.  Citations "P:<line>" are
+ * line numbers of /root/reference/PAPER.md; "R<k>" are the readings listed in DESIGN.md §4 (the
+ * paper prints no formula for its graph and defers to its Ref. [10]).
+ *
+ * Conventions common to every call
+ *   - plain C, no torch types.  Every pointer named d_* is a DEVICE pointer, every pointer named h_*
+ *     is a HOST pointer; both are owned by the caller.  The library never frees, reallocates or keeps
+ *     a caller pointer beyond the call, except the G0 table (borrowed until replaced/destroyed).
+ *   - all floating point is IEEE FP64 (north_star; the paper itself ran FP32, reading R12).
+ *   - calls on d_* buffers are ASYNCHRONOUS on the stream given to cos_create; results are valid
+ *     after the caller synchronises that stream.  Calls on h_* buffers synchronise before returning.
+ *   - return value: COS_OK (0) or a negative cos_status; cos_strerror() gives the text.  No
+ *     exceptions, nothing printed, no global state.  A failed call leaves outputs unspecified.
+ *   - there is NO CPU fallback: every compute entry point needs a CUDA device of compute
+ *     capability 10.x and fails with COS_ECUDA otherwise.
+ *   - batch == 0 is legal everywhere (no work, COS_OK).  n must be in [1, COS_MAX_ORDER].
+ *   - one cos_ctx must not be used from two host threads at once.
+ */
+#ifndef COS_B200_H
+#define COS_B200_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define COS_MAX_ORDER 16
+#define COS_ABI_VERSION 1
+
+typedef enum cos_status {
+    COS_OK = 0,
+    COS_EINVAL = -1,   /* bad argument: n out of range, batch < 0, NULL where not allowed, ntau < 2, ... */
+    COS_ECUDA = -2,    /* CUDA runtime/driver error (no device, launch failure, ...) */
+    COS_ENOMEM = -3,   /* device scratch allocation failed */
+    COS_ENOTABLE = -4  /* a call that needs the G0 table was made before cos_set_g0_table */
+} cos_status;
+
+typedef struct cos_ctx cos_ctx; /* opaque; owns only internal device scratch */
+
+/* Create a context on CUDA device `device`.  `cuda_stream` is a cudaStream_t (e.g. PyTorch's
+ * torch.cuda.current_stream().cuda_stream cast to a pointer); NULL = the legacy default stream.
+ * Allocates no large buffers; scratch grows on demand inside later calls.  *out receives the ctx. */
+int cos_create(cos_ctx** out, int device, void* cuda_stream);
+
+/* Free the context and its scratch (synchronises the stream first).  NULL is COS_EINVAL. */
+int cos_destroy(cos_ctx* ctx);
+
+/* Register the tabulated free propagator G0_s(x, tau) (setup step a0, not timed).
+ *   spin: 0 = up, 1 = down, -1 = both species share this table.
+ *   d_table: DEVICE, FP64, layout [Lx][Ly][ntau] with tau fastest; entry k holds G0 at
+ *            tau_k = k*beta/(ntau-1), k = 0..ntau-1 (end points are 0+ and beta-; reading R8).
+ *   The pointer is BORROWED until replaced or the ctx is destroyed.  Lx, Ly >= 1, ntau >= 2, beta > 0.
+ * (BASELINE.json north_star: "tabulated free propagator G0(x,tau)"; the paper takes G_ab as given.) */
+int cos_set_g0_table(cos_ctx* ctx, int spin, const double* d_table, int Lx, int Ly, int ntau, double beta);
+
+/* Step a1, G assembly for a whole batch (north_star subsystem (a)):
+ *   G_s[b][i][j] = G0_s((x_i - x_j) mod L, tau_i - tau_j) by 2-point linear interpolation in tau,
+ *   antiperiodic in tau:  dtau > 0: lerp(T, dtau);  dtau <= 0 and i != j: -lerp(T, dtau + beta) (R8, R9);
+ *   u = dtau*(ntau-1)/beta, k = min(floor(u), ntau-2), value = fma(u-k, T[k+1]-T[k], T[k]);
+ *   diagonal i == j: g_diag (equal-time convention, reading R7; default of the workloads is 0).
+ *   d_xy : DEVICE int32 [batch][n][2] lattice sites, 0 <= x < Lx, 0 <= y < Ly (not range-checked)
+ *   d_tau: DEVICE FP64  [batch][n], 0 <= tau < beta
+ *   d_Gup, d_Gdn: DEVICE FP64 [batch][n][n] row-major outputs.  d_Gdn may be NULL or equal to d_Gup,
+ *   in which case only the spin-up matrix is written (requires both species to share one table).
+ * Errors: COS_ENOTABLE if a needed table is missing; COS_EINVAL for bad n/batch/NULL. */
+int cos_build_G(cos_ctx* ctx, int n, long long batch, const int* d_xy, const double* d_tau,
+                double g_diag, double* d_Gup, double* d_Gdn);
+
+/* Steps a2+a3 (+a5): sum over ALL diagrams (connected and disconnected) of order n,
+ *   out[b] = prod_a(-u_a) * sum_{sigma_up, sigma_dn} (-1)^{#loops} prod_i Gup[i][sigma_up(i)] Gdn[i][sigma_dn(i)]
+ *          = prod_a(-u_a) * det Gup[b] * det Gdn[b],
+ * computed by the layered (subset, current-vertex) graph, not by LU (top node 1, each edge
+ * multiplies by one Green's function, nodes sum; -1 per closed fermion loop; R1, R6).
+ *   d_Gup, d_Gdn: DEVICE FP64 [batch][n][n] row-major.  d_Gdn == d_Gup (pointer equality) means both
+ *                 species share one matrix: one propagation, D = w * Z^2.
+ *   d_u: DEVICE FP64 [batch][n] per-vertex couplings u_a = V_aa (reading R10), or NULL: every u_a = U.
+ *   d_out: DEVICE FP64 [batch]. */
+int cos_eval_all(cos_ctx* ctx, int n, long long batch, const double* d_Gup, const double* d_Gdn,
+                 const double* d_u, double U, double* d_out);
+
+/* Steps a2+a3+a4 (+a5): the same sum restricted to CONNECTED diagrams ("all connected
+ * diagrams of order n can be summed in O(n^2 2^n) operations"): the permutation pair is kept iff the
+ * graph on the n vertices with edges {i,sigma_up(i)}, {i,sigma_dn(i)} is connected.  Computed as
+ * propagation -> D[S] for every vertex subset -> subset recursion C[S] = D[S] - sum C[T] D[S\T]
+ * (paper's Ref. [9]; north_star subsystem (c); reading R5).  Same arguments as cos_eval_all. */
+int cos_eval_connected(cos_ctx* ctx, int n, long long batch, const double* d_Gup, const double* d_Gdn,
+                       const double* d_u, double U, double* d_out);
+
+/* Fused path a1..a5: vertices in, connected value out; G lives only in library scratch.
+ * Both species use their registered tables; if they share one table a single propagation is done.
+ * Arguments as in cos_build_G / cos_eval_connected. */
+int cos_eval_connected_xt(cos_ctx* ctx, int n, long long batch, const int* d_xy, const double* d_tau,
+                          double g_diag, const double* d_u, double U, double* d_out);
+
+/* The same fused path with HOST buffers (pinned memory recommended): copies h_xy, h_tau (and h_u if
+ * not NULL) to the device, runs a1..a5, copies the batch results back into h_out and synchronises
+ * the stream before returning.  Used for end-to-end timing (h2d = batch*(8n + 8n [+ 8n]) bytes,
+ * d2h = 8*batch bytes). */
+int cos_eval_connected_xt_host(cos_ctx* ctx, int n, long long batch, const int* h_xy,
+                               const double* h_tau, double g_diag, const double* h_u, double U,
+                               double* h_out);
+
+/* Number of kernel launches issued by the most recent compute call on this ctx (>= 1 on success). */
+int cos_last_launch_count(const cos_ctx* ctx);
+
+/* Name of the dominant kernel variant the most recent eval call dispatched to (static string). */
+const char* cos_last_kernel_name(const cos_ctx* ctx);
+
+/* Average duration in milliseconds of the dominant (evaluation) kernel over the launches issued by
+ * this ctx since the last cos_reset_kernel_timer(), measured with CUDA events recorded on the ctx
+ * stream around that kernel only.  Timing is off by default (zero overhead); enable != 0 switches it
+ * on.  cos_kernel_time_ms synchronises the stream.  Returns COS_EINVAL if nothing was timed. */
+int cos_enable_kernel_timer(cos_ctx* ctx, int enable);
+int cos_reset_kernel_timer(cos_ctx* ctx);
+int cos_kernel_time_ms(cos_ctx* ctx, double* avg_ms, long long* launches);
+
+/* Algorithmic operation count per configuration (1 FMA = 2 FLOP; no GPU needed):
+ *   ext(n) = (n^2-3n+4) 2^(n-2) - 1 extend FMAs and close(n) = n 2^(n-1) close FMAs per species,
+ *   2^n combine multiplies, red(n) = 3^(n-1) - 2^(n-1) reduction FMAs (connected only).
+ * n_species = 1 (aliased) or 2.  Returns FLOP per configuration, or -1 for bad arguments. */
+long long cos_flop_count(int n, int n_species, int connected);
+
+/* Roofline denominators measured on the device of this ctx (synchronous, a few milliseconds each):
+ *   cos_probe_dfma:  sustained FP64 FMA throughput of a register-only kernel, in TFLOP/s;
+ *   cos_probe_smem:  sustained shared-memory load bandwidth (conflict-free LDS.64), in GB/s. */
+int cos_probe_dfma(cos_ctx* ctx, double* tflops);
+int cos_probe_smem(cos_ctx* ctx, double* gbytes_per_s);
+
+/* Text for a status code (never NULL).  For COS_ECUDA, cos_last_cuda_error gives the CUDA text. */
+const char* cos_strerror(int code);
+const char* cos_last_cuda_error(const cos_ctx* ctx);
+
+int cos_abi_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* COS_B200_H */

@@ -1,0 +1,373 @@
+// cos_api.cu -- C-ABI entry points of libcos_b200.so (include/cos.h): context, argument validation,
+// scratch management, kernel dispatch.  Host code only touches pointers and sizes; every step of the
+// path (a1..a5) runs in the kernels.  There is no CPU fallback.
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "cos_common.cuh"
+#include "cos_kernels_generic.cuh"
+#include "cos_dispatch.cuh"
+
+using namespace cosb;
+
+struct cos_ctx {
+    int device = 0;
+    cudaStream_t stream = nullptr;
+    int num_sms = 0;
+    int smem_optin = 0;
+    // G0 tables (borrowed)
+    const double* table[2] = {nullptr, nullptr};
+    int Lx = 0, Ly = 0, ntau = 0;
+    double beta = 0.0;
+    // scratch (owned)
+    uint32_t* off = nullptr;
+    double* scratch = nullptr;      size_t scratch_bytes = 0;
+    double* gscratch = nullptr;     size_t gscratch_bytes = 0;   // G matrices of the fused path
+    void* stage = nullptr;          size_t stage_bytes = 0;      // device staging of the host path
+    // bookkeeping
+    int last_launches = 0;
+    const char* last_kernel = "none";
+    cudaError_t last_err = cudaSuccess;
+    // optional timing of the evaluation kernel
+    bool timing = false;
+    std::vector<cudaEvent_t> ev;    // pairs (start, stop)
+    size_t ev_used = 0;
+};
+
+namespace {
+
+int fail_cuda(cos_ctx* c, cudaError_t e)
+{
+    if (c) c->last_err = e;
+    return COS_ECUDA;
+}
+
+#define COS_CUDA(c, expr)                                   \
+    do {                                                    \
+        cudaError_t e__ = (expr);                           \
+        if (e__ != cudaSuccess) return fail_cuda((c), e__); \
+    } while (0)
+
+int grow(cos_ctx* c, void** p, size_t* have, size_t need)
+{
+    if (need <= *have) return COS_OK;
+    if (*p) {
+        COS_CUDA(c, cudaStreamSynchronize(c->stream));
+        cudaFree(*p);
+        *p = nullptr;
+        *have = 0;
+    }
+    cudaError_t e = cudaMalloc(p, need);
+    if (e != cudaSuccess) { c->last_err = e; (void)cudaGetLastError(); return COS_ENOMEM; }
+    *have = need;
+    return COS_OK;
+}
+
+bool timer_begin(cos_ctx* c)
+{
+    if (!c->timing) return false;
+    if (c->ev_used + 2 > c->ev.size()) {
+        for (int k = 0; k < 2; ++k) {
+            cudaEvent_t e;
+            if (cudaEventCreate(&e) != cudaSuccess) return false;
+            c->ev.push_back(e);
+        }
+    }
+    cudaEventRecord(c->ev[c->ev_used], c->stream);
+    return true;
+}
+void timer_end(cos_ctx* c)
+{
+    cudaEventRecord(c->ev[c->ev_used + 1], c->stream);
+    c->ev_used += 2;
+}
+
+int check_eval_args(cos_ctx* c, int n, long long batch, const void* gup, const void* gdn, const void* out)
+{
+    if (!c) return COS_EINVAL;
+    if (n < 1 || n > COS_MAX_ORDER || batch < 0) return COS_EINVAL;
+    if (batch > 0 && (!gup || !gdn || !out)) return COS_EINVAL;
+    return COS_OK;
+}
+
+int launch_eval(cos_ctx* c, const EvalArgs& args)
+{
+    const bool t = timer_begin(c);
+    int launches = 0;
+    const char* name = nullptr;
+    cudaError_t e = dispatch_eval(args, c->stream, c->num_sms, c->smem_optin, &launches, &name);
+    if (t) timer_end(c);
+    if (e != cudaSuccess) return fail_cuda(c, e);
+    c->last_launches += launches;
+    c->last_kernel = name;
+    return COS_OK;
+}
+
+int do_eval(cos_ctx* c, int n, long long batch, const double* gup, const double* gdn, const double* u,
+            double U, double* out, int connected)
+{
+    if (batch == 0) return COS_OK;
+    EvalArgs a{};
+    a.n = n; a.batch = batch; a.Gup = gup; a.Gdn = gdn; a.u = u; a.U = U; a.out = out;
+    a.connected = connected; a.off = c->off;
+    // global scratch for the orders whose frontier does not fit in shared memory
+    const size_t per_cta = eval_scratch_doubles(n, c->smem_optin);
+    if (per_cta) {
+        const int ctas = eval_max_ctas(n, batch, c->num_sms, c->smem_optin);
+        int rc = grow(c, (void**)&c->scratch, &c->scratch_bytes, per_cta * sizeof(double) * (size_t)ctas);
+        if (rc != COS_OK) return rc;
+        a.scratch = c->scratch;
+        a.scratch_stride = per_cta;
+    }
+    return launch_eval(c, a);
+}
+
+int do_build_G(cos_ctx* c, int n, long long batch, const int* xy, const double* tau, double g_diag,
+               double* gup, double* gdn)
+{
+    if (batch == 0) return COS_OK;
+    BuildGArgs a{};
+    a.n = n; a.batch = batch; a.xy = xy; a.tau = tau;
+    a.Tup = c->table[0]; a.Tdn = c->table[1];
+    a.Lx = c->Lx; a.Ly = c->Ly; a.ntau = c->ntau; a.beta = c->beta; a.g_diag = g_diag;
+    a.Gup = gup; a.Gdn = (gdn == gup) ? nullptr : gdn;
+    const long long total = batch * n * n;
+    long long blocks = (total + 255) / 256;
+    const long long cap = (long long)c->num_sms * 16;
+    if (blocks > cap) blocks = cap;
+    build_G_kernel<<<(unsigned)blocks, 256, 0, c->stream>>>(a);
+    COS_CUDA(c, cudaGetLastError());
+    c->last_launches += 1;
+    return COS_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int cos_abi_version(void) { return COS_ABI_VERSION; }
+
+const char* cos_strerror(int code)
+{
+    switch (code) {
+        case COS_OK: return "success";
+        case COS_EINVAL: return "invalid argument";
+        case COS_ECUDA: return "CUDA error (see cos_last_cuda_error)";
+        case COS_ENOMEM: return "device scratch allocation failed";
+        case COS_ENOTABLE: return "G0 table not set (call cos_set_g0_table first)";
+        default: return "unknown status";
+    }
+}
+
+const char* cos_last_cuda_error(const cos_ctx* ctx)
+{
+    return ctx ? cudaGetErrorString(ctx->last_err) : "no context";
+}
+
+int cos_create(cos_ctx** out, int device, void* cuda_stream)
+{
+    if (!out) return COS_EINVAL;
+    *out = nullptr;
+    int count = 0;
+    if (cudaGetDeviceCount(&count) != cudaSuccess || device < 0 || device >= count) {
+        (void)cudaGetLastError();
+        return COS_ECUDA;
+    }
+    cos_ctx* c = new (std::nothrow) cos_ctx();
+    if (!c) return COS_ENOMEM;
+    c->device = device;
+    c->stream = (cudaStream_t)cuda_stream;
+    cudaDeviceProp prop;
+    if (cudaSetDevice(device) != cudaSuccess || cudaGetDeviceProperties(&prop, device) != cudaSuccess) {
+        delete c;
+        return COS_ECUDA;
+    }
+    if (prop.major != 10) {   // sm_100a only: no multi-backend dispatch, no fallback
+        delete c;
+        return COS_ECUDA;
+    }
+    c->num_sms = prop.multiProcessorCount;
+    c->smem_optin = (int)prop.sharedMemPerBlockOptin;
+    const uint32_t count_off = 1u << (COS_MAX_ORDER - 1);
+    if (cudaMalloc((void**)&c->off, sizeof(uint32_t) * (count_off + 1)) != cudaSuccess) {
+        delete c;
+        return COS_ENOMEM;
+    }
+    init_off_table_kernel<<<1, 1024, 0, c->stream>>>(c->off, count_off + 1);
+    cudaError_t e = configure_kernels(c->smem_optin);
+    if (e == cudaSuccess) e = cudaGetLastError();
+    if (e != cudaSuccess) {
+        cudaFree(c->off);
+        delete c;
+        return COS_ECUDA;
+    }
+    *out = c;
+    return COS_OK;
+}
+
+int cos_destroy(cos_ctx* c)
+{
+    if (!c) return COS_EINVAL;
+    cudaSetDevice(c->device);
+    cudaStreamSynchronize(c->stream);
+    for (cudaEvent_t e : c->ev) cudaEventDestroy(e);
+    cudaFree(c->off);
+    cudaFree(c->scratch);
+    cudaFree(c->gscratch);
+    cudaFree(c->stage);
+    delete c;
+    return COS_OK;
+}
+
+int cos_set_g0_table(cos_ctx* c, int spin, const double* d_table, int Lx, int Ly, int ntau, double beta)
+{
+    if (!c || !d_table || spin < -1 || spin > 1 || Lx < 1 || Ly < 1 || ntau < 2 || !(beta > 0.0)) return COS_EINVAL;
+    const bool other_set = (spin >= 0) && c->table[1 - spin] != nullptr;
+    if (other_set && (Lx != c->Lx || Ly != c->Ly || ntau != c->ntau || beta != c->beta)) return COS_EINVAL;
+    if (spin == -1) c->table[0] = c->table[1] = d_table;
+    else c->table[spin] = d_table;
+    c->Lx = Lx; c->Ly = Ly; c->ntau = ntau; c->beta = beta;
+    return COS_OK;
+}
+
+int cos_build_G(cos_ctx* c, int n, long long batch, const int* d_xy, const double* d_tau, double g_diag,
+                double* d_Gup, double* d_Gdn)
+{
+    if (!c || n < 1 || n > COS_MAX_ORDER || batch < 0) return COS_EINVAL;
+    if (batch > 0 && (!d_xy || !d_tau || !d_Gup)) return COS_EINVAL;
+    if (!c->table[0]) return COS_ENOTABLE;
+    const bool single = (d_Gdn == nullptr || d_Gdn == d_Gup);
+    if (!single && !c->table[1]) return COS_ENOTABLE;
+    if (single && c->table[1] && c->table[1] != c->table[0]) return COS_EINVAL;  // one output, two tables
+    cudaSetDevice(c->device);
+    c->last_launches = 0;
+    return do_build_G(c, n, batch, d_xy, d_tau, g_diag, d_Gup, single ? d_Gup : d_Gdn);
+}
+
+int cos_eval_all(cos_ctx* c, int n, long long batch, const double* d_Gup, const double* d_Gdn,
+                 const double* d_u, double U, double* d_out)
+{
+    int rc = check_eval_args(c, n, batch, d_Gup, d_Gdn, d_out);
+    if (rc != COS_OK) return rc;
+    cudaSetDevice(c->device);
+    c->last_launches = 0;
+    return do_eval(c, n, batch, d_Gup, d_Gdn, d_u, U, d_out, 0);
+}
+
+int cos_eval_connected(cos_ctx* c, int n, long long batch, const double* d_Gup, const double* d_Gdn,
+                       const double* d_u, double U, double* d_out)
+{
+    int rc = check_eval_args(c, n, batch, d_Gup, d_Gdn, d_out);
+    if (rc != COS_OK) return rc;
+    cudaSetDevice(c->device);
+    c->last_launches = 0;
+    return do_eval(c, n, batch, d_Gup, d_Gdn, d_u, U, d_out, 1);
+}
+
+int cos_eval_connected_xt(cos_ctx* c, int n, long long batch, const int* d_xy, const double* d_tau,
+                          double g_diag, const double* d_u, double U, double* d_out)
+{
+    if (!c || n < 1 || n > COS_MAX_ORDER || batch < 0) return COS_EINVAL;
+    if (batch > 0 && (!d_xy || !d_tau || !d_out)) return COS_EINVAL;
+    if (!c->table[0]) return COS_ENOTABLE;
+    cudaSetDevice(c->device);
+    c->last_launches = 0;
+    if (batch == 0) return COS_OK;
+    const bool two = c->table[1] && c->table[1] != c->table[0];
+    const size_t one = (size_t)batch * n * n * sizeof(double);
+    int rc = grow(c, (void**)&c->gscratch, &c->gscratch_bytes, two ? 2 * one : one);
+    if (rc != COS_OK) return rc;
+    double* gup = c->gscratch;
+    double* gdn = two ? c->gscratch + (size_t)batch * n * n : gup;
+    rc = do_build_G(c, n, batch, d_xy, d_tau, g_diag, gup, gdn);
+    if (rc != COS_OK) return rc;
+    return do_eval(c, n, batch, gup, gdn, d_u, U, d_out, 1);
+}
+
+int cos_eval_connected_xt_host(cos_ctx* c, int n, long long batch, const int* h_xy, const double* h_tau,
+                               double g_diag, const double* h_u, double U, double* h_out)
+{
+    if (!c || n < 1 || n > COS_MAX_ORDER || batch < 0) return COS_EINVAL;
+    if (batch > 0 && (!h_xy || !h_tau || !h_out)) return COS_EINVAL;
+    if (!c->table[0]) return COS_ENOTABLE;
+    cudaSetDevice(c->device);
+    c->last_launches = 0;
+    if (batch == 0) return COS_OK;
+    const size_t b_xy = (size_t)batch * n * 2 * sizeof(int);
+    const size_t b_tau = (size_t)batch * n * sizeof(double);
+    const size_t b_u = h_u ? b_tau : 0;
+    const size_t b_out = (size_t)batch * sizeof(double);
+    int rc = grow(c, &c->stage, &c->stage_bytes, b_xy + b_tau + b_u + b_out);
+    if (rc != COS_OK) return rc;
+    char* base = (char*)c->stage;
+    double* d_tau = (double*)base;
+    double* d_u = h_u ? (double*)(base + b_tau) : nullptr;
+    double* d_out = (double*)(base + b_tau + b_u);
+    int* d_xy = (int*)(base + b_tau + b_u + b_out);
+    COS_CUDA(c, cudaMemcpyAsync(d_xy, h_xy, b_xy, cudaMemcpyHostToDevice, c->stream));
+    COS_CUDA(c, cudaMemcpyAsync(d_tau, h_tau, b_tau, cudaMemcpyHostToDevice, c->stream));
+    if (h_u) COS_CUDA(c, cudaMemcpyAsync(d_u, h_u, b_u, cudaMemcpyHostToDevice, c->stream));
+    const int saved = c->last_launches;
+    rc = cos_eval_connected_xt(c, n, batch, d_xy, d_tau, g_diag, d_u, U, d_out);
+    (void)saved;
+    if (rc != COS_OK) return rc;
+    COS_CUDA(c, cudaMemcpyAsync(h_out, d_out, b_out, cudaMemcpyDeviceToHost, c->stream));
+    COS_CUDA(c, cudaStreamSynchronize(c->stream));
+    return COS_OK;
+}
+
+int cos_last_launch_count(const cos_ctx* c) { return c ? c->last_launches : 0; }
+const char* cos_last_kernel_name(const cos_ctx* c) { return c ? c->last_kernel : "none"; }
+
+int cos_enable_kernel_timer(cos_ctx* c, int enable)
+{
+    if (!c) return COS_EINVAL;
+    c->timing = enable != 0;
+    return COS_OK;
+}
+
+int cos_reset_kernel_timer(cos_ctx* c)
+{
+    if (!c) return COS_EINVAL;
+    c->ev_used = 0;
+    return COS_OK;
+}
+
+int cos_kernel_time_ms(cos_ctx* c, double* avg_ms, long long* launches)
+{
+    if (!c || !avg_ms || c->ev_used == 0) return COS_EINVAL;
+    cudaSetDevice(c->device);
+    COS_CUDA(c, cudaStreamSynchronize(c->stream));
+    double total = 0.0;
+    for (size_t k = 0; k < c->ev_used; k += 2) {
+        float ms = 0.f;
+        COS_CUDA(c, cudaEventElapsedTime(&ms, c->ev[k], c->ev[k + 1]));
+        total += ms;
+    }
+    *avg_ms = total / (double)(c->ev_used / 2);
+    if (launches) *launches = (long long)(c->ev_used / 2);
+    return COS_OK;
+}
+
+long long cos_flop_count(int n, int n_species, int connected)
+{
+    if (n < 1 || n > 20 || n_species < 1 || n_species > 2) return -1;
+    const long long two_n = 1LL << n;
+    // ext(n) = (n^2-3n+4) 2^(n-2) - 1 ; close(n) = n 2^(n-1)   (exact for n >= 1; n = 1: ext = 0)
+    const long long ext = ((long long)(n * n - 3 * n + 4) * two_n) / 4 - 1;
+    const long long close = (long long)n * two_n / 2;
+    long long fma_total = n_species * (ext + close);
+    long long flop = 2 * fma_total;
+    if (connected) {
+        long long p3 = 1;
+        for (int i = 0; i < n - 1; ++i) p3 *= 3;
+        flop += 2 * (p3 - two_n / 2);       // reduction FMAs
+        flop += 2 * two_n;                   // combine: 2^n entries, counted like an FMA each
+    }
+    return flop;
+}
+
+}  // extern "C"

@@ -1,0 +1,225 @@
+// cos_kernels_generic.cuh -- generic (any n in 1..16) CoS evaluation kernel and the G-assembly kernel.
+//
+// This is the reference-correct CUDA path: one CTA per configuration, grid-strided over the batch,
+// the whole path a2..a5 inside one kernel.  It is the fallback for orders that have no specialised
+// kernel and the kernel every specialised variant is tested against (besides the oracle).
+//
+// Method (reading R1):
+//   nodes (S, c): S = vertex subset, c in S = current end of the open path that started at h(S) = max S.
+//   Organised by "stage" h = h(S): stage h works on R = S \ {h}, R subset of [h] = {0..h-1}:
+//       P_h[R][h]  = Z[R]                                            (start a loop at h)
+//       P_h[R+c'][c'] = sum_{c in R+{h}} P_h[R][c] * W[c][c']  c' not in R   (extend)
+//       Z[R+{h}]   = - sum_{c in R+{h}} P_h[R][c] * W[c][h]          (close, -1 per fermion loop)
+//   levels j = |R| = 0..h are processed in sequence with a block barrier, stages in sequence
+//   because stage h reads every Z[R], R subset of [h].  Z[S] = (-1)^|S| det W[S,S] for every S.
+//   Then D[S] = w(S) Zup[S] Zdn[S] and the subset recursion for the connected part.
+#pragma once
+#include "cos_common.cuh"
+
+namespace cosb {
+
+// ------------------------------------------------------------------------------------------ a1
+// One thread per (b, i, j).  Table rows are L2 resident (1-8 MiB); two adjacent tau points per entry.
+__global__ void __launch_bounds__(256) build_G_kernel(BuildGArgs a)
+{
+    const long long total = a.batch * a.n * a.n;
+    for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < total;
+         t += (long long)gridDim.x * blockDim.x) {
+        const int j = (int)(t % a.n);
+        const long long bi = t / a.n;
+        const int i = (int)(bi % a.n);
+        const long long b = bi / a.n;
+        if (i == j) {
+            a.Gup[t] = a.g_diag;
+            if (a.Gdn) a.Gdn[t] = a.g_diag;
+            continue;
+        }
+        const int* pi = a.xy + (b * a.n + i) * 2;
+        const int* pj = a.xy + (b * a.n + j) * 2;
+        int dx = (pi[0] - pj[0]) % a.Lx; if (dx < 0) dx += a.Lx;
+        int dy = (pi[1] - pj[1]) % a.Ly; if (dy < 0) dy += a.Ly;
+        double dtau = a.tau[b * a.n + i] - a.tau[b * a.n + j];
+        double sign = 1.0;
+        if (dtau <= 0.0) { dtau = __dadd_rn(dtau, a.beta); sign = -1.0; }     // R9: dtau == 0 is 0-
+        const double uu = __ddiv_rn(__dmul_rn(dtau, (double)(a.ntau - 1)), a.beta);
+        int k = (int)floor(uu);
+        k = min(k, a.ntau - 2);
+        k = max(k, 0);
+        const double f = __dsub_rn(uu, (double)k);
+        const size_t row = ((size_t)dx * a.Ly + dy) * (size_t)a.ntau + k;
+        {
+            const double t0 = __ldg(a.Tup + row), t1 = __ldg(a.Tup + row + 1);
+            a.Gup[t] = sign * __fma_rn(f, __dsub_rn(t1, t0), t0);
+        }
+        if (a.Gdn) {
+            const double t0 = __ldg(a.Tdn + row), t1 = __ldg(a.Tdn + row + 1);
+            a.Gdn[t] = sign * __fma_rn(f, __dsub_rn(t1, t0), t0);
+        }
+    }
+}
+
+// off[R] = sum_{x<R} (popc(x)+1): slot of node (R, first element) when the nodes of one stage are
+// stored in numeric order of R, each R holding popc(R)+1 values (elements of R ascending, then h).
+__global__ void init_off_table_kernel(uint32_t* off, uint32_t count)
+{
+    // single block, serial prefix per thread chunk is unnecessary: count <= 32769, do a simple scan.
+    __shared__ uint32_t partial[1024];
+    const uint32_t per = (count + blockDim.x - 1) / blockDim.x;
+    const uint32_t lo = threadIdx.x * per, hi = min(count, lo + per);
+    uint32_t s = 0;
+    for (uint32_t x = lo; x < hi; ++x) s += __popc(x) + 1;
+    partial[threadIdx.x] = s;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        uint32_t run = 0;
+        for (unsigned t = 0; t < blockDim.x; ++t) { const uint32_t v = partial[t]; partial[t] = run; run += v; }
+    }
+    __syncthreads();
+    s = partial[threadIdx.x];
+    for (uint32_t x = lo; x < hi; ++x) { off[x] = s; s += __popc(x) + 1; }
+}
+
+// Shared-memory footprint of the generic kernel, in doubles.
+//   W: 2*n*n, u: n (padded to 16), Z: nsp * 2^n, P: (n+1) 2^(n-2) (stage n-1; also holds C' later)
+__host__ __device__ inline size_t generic_frontier_doubles(int n)
+{
+    return n >= 2 ? ((size_t)(n + 1) << (n - 2)) : 2;
+}
+__host__ __device__ inline size_t generic_small_doubles(int n) { return (size_t)2 * n * n + 16; }
+
+template <int kThreads>
+__global__ void __launch_bounds__(kThreads) eval_generic_kernel(EvalArgs a, int nsp, int use_global)
+{
+    extern __shared__ double smem[];
+    const int n = a.n;
+    const int tid = threadIdx.x;
+    const unsigned N = 1u << n;
+    double* W = smem;                       // [nsp][n][n]
+    double* uvec = smem + 2 * n * n;        // [n] (-u_a)
+    double* Z;                              // [nsp][N]
+    double* P;                              // frontier of the current stage / C' in the reduction
+    if (use_global) {
+        Z = a.scratch + (size_t)blockIdx.x * a.scratch_stride;
+        P = Z + (size_t)2 * N;
+    } else {
+        Z = smem + generic_small_doubles(n);
+        P = Z + (size_t)nsp * N;
+    }
+    const uint32_t* __restrict__ off = a.off;
+
+    for (long long b = blockIdx.x; b < a.batch; b += gridDim.x) {
+        __syncthreads();
+        // ---- load W (both species) and the couplings; fold -u_a into the rows of W_up when the
+        //      species are distinct (each term has exactly one factor from every row of S) ----
+        for (int t = tid; t < n; t += kThreads) uvec[t] = -(a.u ? a.u[b * n + t] : a.U);
+        __syncthreads();
+        for (int t = tid; t < n * n; t += kThreads) {
+            const double g = a.Gup[b * n * n + t];
+            W[t] = (nsp == 2) ? g * uvec[t / n] : g;
+            if (nsp == 2) W[n * n + t] = a.Gdn[b * n * n + t];
+        }
+        __syncthreads();
+
+        // ---- a2: propagation, one species after the other ----
+        for (int s = 0; s < nsp; ++s) {
+            const double* Ws = W + s * n * n;
+            double* Zs = Z + (size_t)s * N;
+            if (tid == 0) Zs[0] = 1.0;                      // top node = 1
+            __syncthreads();
+            for (int h = 0; h < n; ++h) {
+                const unsigned NR = 1u << h;
+                for (unsigned R = tid; R < NR; R += kThreads)   // start: P_h[R][h] = Z[R]
+                    P[off[R] + __popc(R)] = Zs[R];
+                __syncthreads();
+                for (int j = 0; j <= h; ++j) {
+                    for (unsigned R = tid; R < NR; R += kThreads) {
+                        if (__popc(R) != j) continue;
+                        const double* pr = P + off[R];
+                        const double ah = pr[j];
+                        // close: Z[R + {h}] = - sum_c P[R][c] W[c][h]
+                        {
+                            double acc = ah * Ws[h * n + h];
+                            unsigned m = R; int i = 0;
+                            while (m) { const int c = __ffs(m) - 1; m &= m - 1; acc = fma(pr[i++], Ws[c * n + h], acc); }
+                            Zs[R | NR] = -acc;
+                        }
+                        // extend to every c' < h not in R
+                        unsigned absent = ~R & (NR - 1);
+                        while (absent) {
+                            const int cp = __ffs(absent) - 1; absent &= absent - 1;
+                            double acc = ah * Ws[h * n + cp];
+                            unsigned m = R; int i = 0;
+                            while (m) { const int c = __ffs(m) - 1; m &= m - 1; acc = fma(pr[i++], Ws[c * n + cp], acc); }
+                            const unsigned R2 = R | (1u << cp);
+                            P[off[R2] + __popc(R2 & ((1u << cp) - 1))] = acc;
+                        }
+                    }
+                    __syncthreads();
+                }
+            }
+        }
+
+        const double* Zup = Z;
+        const double* Zdn = Z + (size_t)(nsp - 1) * N;
+        if (!a.connected) {                                  // a5 "all": D[full]
+            if (tid == 0) {
+                double w = 1.0;
+                if (nsp == 1) for (int v = 0; v < n; ++v) w *= uvec[v];
+                a.out[b] = w * Zup[N - 1] * Zdn[N - 1];
+            }
+            continue;
+        }
+
+        // ---- a3: D[S] = w(S) Zup[S] Zdn[S], stored over Zup ----
+        double* D = Z;
+        for (unsigned S = tid; S < N; S += kThreads) {
+            double w = 1.0;
+            if (nsp == 1) { unsigned m = S; while (m) { const int v = __ffs(m) - 1; m &= m - 1; w *= uvec[v]; } }
+            D[S] = w * Zup[S] * Zdn[S];
+        }
+        __syncthreads();
+
+        // ---- a4: C'[S'] = D[2S'+1] - sum_{T' proper subset of S'} C'[T'] D[2(S'\T')], levels |S'| ----
+        double* C = P;
+        const unsigned M = N >> 1;                           // subsets of vertices 1..n-1
+        const int lane = tid & 31, warp = tid >> 5, nwarps = kThreads >> 5;
+        for (int l = 0; l < n; ++l) {
+            if (l < 5) {
+                for (unsigned Sp = tid; Sp < M; Sp += kThreads) {
+                    if (__popc(Sp) != l) continue;
+                    double acc = D[2 * Sp + 1];
+                    for (unsigned Tp = (Sp - 1) & Sp; Sp != 0; Tp = (Tp - 1) & Sp) {
+                        acc = fma(-C[Tp], D[2 * (Sp ^ Tp)], acc);
+                        if (Tp == 0) break;
+                    }
+                    C[Sp] = acc;
+                }
+            } else {
+                // one warp per output; lanes own the 32 sub-subsets of the 5 lowest vertices of S'
+                for (unsigned Sp = warp; Sp < M; Sp += nwarps) {
+                    if (__popc(Sp) != l) continue;
+                    unsigned low5 = 0, tlo = 0, m = Sp;
+                    for (int q = 0; q < 5; ++q) {
+                        const unsigned bit = m & (0u - m); m ^= bit; low5 |= bit;
+                        if (lane >> q & 1) tlo |= bit;
+                    }
+                    const unsigned Shi = Sp ^ low5;
+                    double acc = 0.0;
+                    unsigned Thi = Shi;
+                    while (true) {
+                        const unsigned Tp = Thi | tlo;
+                        if (Tp != Sp) acc = fma(C[Tp], D[2 * (Sp ^ Tp)], acc);
+                        if (Thi == 0) break;
+                        Thi = (Thi - 1) & Shi;
+                    }
+                    for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+                    if (lane == 0) C[Sp] = D[2 * Sp + 1] - acc;
+                }
+            }
+            __syncthreads();
+        }
+        if (tid == 0) a.out[b] = C[M - 1];
+    }
+}
+
+}  // namespace cosb

@@ -1,0 +1,174 @@
+"""GPU parity tests: the CUDA path, called through the C-ABI binding, against the CPU oracle element by
+element on the same seeded inputs.  Every test here needs a B200 (`-m gpu`).  Tolerances: G assembly
+bit-exact (same FP64 operations in the same order, one explicit fma); evaluation by the rule in
+tests/parity_util.py (1e-10 relative, conditioning-aware exceptions)."""
+import numpy as np
+import pytest
+
+from parity_util import check_parity
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def torch_mod():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("GPU test selected but no CUDA device: the CUDA path has no CPU fallback")
+    return torch
+
+
+@pytest.fixture(scope="module")
+def ctx(torch_mod):
+    from paper_2501_00675_b200 import api
+    c = api.Context()
+    yield c
+    c.close()
+
+
+def _dev(torch, a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def _gpu_eval(torch, ctx, Gup, Gdn, U, u, which):
+    dGup = _dev(torch, Gup)
+    dGdn = dGup if Gdn is None else _dev(torch, Gdn)
+    du = None if u is None else _dev(torch, u)
+    out = torch.empty(Gup.shape[0], dtype=torch.float64, device="cuda")
+    fn = ctx.eval_all if which == "all" else ctx.eval_connected
+    fn(dGup, dGdn, out, U=U, d_u=du)
+    torch.cuda.synchronize()
+    assert ctx.last_launch_count() >= 1
+    return out.cpu().numpy()
+
+
+def _workload_mats(oracle_mod, w):
+    if w.kind == "hubbard":
+        Gup, _ = oracle_mod.build_G(w.xy, w.tau, w.table, None, w.beta, w.g_diag)
+        return Gup, None, w.U, None
+    return w.G, None, w.U, w.u
+
+
+# ------------------------------------------------------------------------------------------ a1
+@pytest.mark.parametrize("cfg,batch", [(1, 64), (2, 4096), (3, 2048), (4, 1024)])
+def test_build_G_bit_exact(torch_mod, ctx, oracle_mod, cfg, batch):
+    from paper_2501_00675_b200 import workloads as wl
+    torch = torch_mod
+    w = wl.baseline_config(cfg, batch=batch)
+    ref_up, ref_dn = oracle_mod.build_G(w.xy, w.tau, w.table, None, w.beta, 0.0)
+    ctx.set_g0_table(_dev(torch, w.table), w.beta)
+    Gup = torch.empty((batch, w.n, w.n), dtype=torch.float64, device="cuda")
+    ctx.build_G(_dev(torch, w.xy), _dev(torch, w.tau), Gup, None, g_diag=0.0)
+    torch.cuda.synchronize()
+    np.testing.assert_array_equal(Gup.cpu().numpy(), ref_up)
+
+
+def test_build_G_two_tables_diag_and_ragged(torch_mod, ctx, oracle_mod):
+    torch = torch_mod
+    rng = np.random.default_rng(0)
+    L, ntau, beta, B, n = 7, 33, 3.7, 37, 5          # odd sizes: ragged tail of the thread grid
+    Tu, Td = rng.normal(size=(L, L, ntau)), rng.normal(size=(L, L, ntau))
+    xy = rng.integers(0, L, size=(B, n, 2)).astype(np.int32)
+    tau = rng.uniform(0, beta, size=(B, n))
+    tau[3, 1] = tau[3, 4]                            # equal times: R9 negative branch
+    ref_up, ref_dn = oracle_mod.build_G(xy, tau, Tu, Td, beta, 0.25)
+    from paper_2501_00675_b200 import api
+    with api.Context() as c2:
+        c2.set_g0_table(_dev(torch, Tu), beta, spin=0)
+        c2.set_g0_table(_dev(torch, Td), beta, spin=1)
+        Gup = torch.empty((B, n, n), dtype=torch.float64, device="cuda")
+        Gdn = torch.empty((B, n, n), dtype=torch.float64, device="cuda")
+        c2.build_G(_dev(torch, xy), _dev(torch, tau), Gup, Gdn, g_diag=0.25)
+        torch.cuda.synchronize()
+        np.testing.assert_array_equal(Gup.cpu().numpy(), ref_up)
+        np.testing.assert_array_equal(Gdn.cpu().numpy(), ref_dn)
+
+
+# ------------------------------------------------------------------------------------------ a2..a5
+@pytest.mark.parametrize("n", list(range(1, 17)))
+def test_eval_every_order_dense(torch_mod, ctx, oracle_mod, n):
+    """Every order 1..16, two distinct species with per-vertex couplings, and the aliased form."""
+    rng = np.random.default_rng(1000 + n)
+    B = 37 if n <= 12 else (9 if n <= 14 else 3)     # ragged, spans several CTAs
+    Gup = rng.normal(size=(B, n, n)) / np.sqrt(n) + 0.5 * np.eye(n)
+    Gdn = rng.normal(size=(B, n, n)) / np.sqrt(n) + 0.5 * np.eye(n)
+    u = rng.uniform(0.5, 2.0, size=(B, n))
+    for which in ("all", "connected"):
+        got = _gpu_eval(torch_mod, ctx, Gup, Gdn, 1.0, u, which)
+        check_parity(oracle_mod, got, Gup, Gdn, 1.0, u, which)
+        got = _gpu_eval(torch_mod, ctx, Gup, None, 1.7, None, which)
+        check_parity(oracle_mod, got, Gup, None, 1.7, None, which)
+
+
+@pytest.mark.parametrize("cfg,batch", [(1, 64), (2, 4096), (3, 1024), (4, 256), (5, 16)])
+def test_eval_baseline_configs(torch_mod, ctx, oracle_mod, cfg, batch):
+    """BASELINE.json configs (sizes the oracle finishes in seconds), element by element."""
+    from paper_2501_00675_b200 import workloads as wl
+    w = wl.baseline_config(cfg, batch=batch)
+    Gup, Gdn, U, u = _workload_mats(oracle_mod, w)
+    for which in ("all", "connected"):
+        got = _gpu_eval(torch_mod, ctx, Gup, Gdn, U, u, which)
+        st = check_parity(oracle_mod, got, Gup, Gdn, U, u, which)
+        print(f"cfg{cfg} {which}: {st}")
+    # two-propagation form of the same Hubbard input (separate copy of G_down) gives the same numbers
+    if w.kind == "hubbard":
+        got2 = _gpu_eval(torch_mod, ctx, Gup, Gup.copy(), U, None, "connected")
+        check_parity(oracle_mod, got2, Gup, Gup.copy(), U, None, "connected")
+
+
+def test_fused_xt_and_host_paths(torch_mod, ctx, oracle_mod):
+    from paper_2501_00675_b200 import workloads as wl
+    torch = torch_mod
+    w = wl.baseline_config(3, batch=300)
+    Gup, _ = oracle_mod.build_G(w.xy, w.tau, w.table, None, w.beta, 0.0)
+    ctx.set_g0_table(_dev(torch, w.table), w.beta)
+    out = torch.empty(w.batch, dtype=torch.float64, device="cuda")
+    ctx.eval_connected_xt(_dev(torch, w.xy), _dev(torch, w.tau), out, U=w.U)
+    torch.cuda.synchronize()
+    assert ctx.last_launch_count() >= 2
+    check_parity(oracle_mod, out.cpu().numpy(), Gup, None, w.U, None, "connected")
+    h_out = np.empty(w.batch)
+    ctx.eval_connected_xt_host(w.xy, w.tau, h_out, U=w.U)
+    np.testing.assert_array_equal(h_out, out.cpu().numpy())
+
+
+def test_degenerate_inputs(torch_mod, ctx, oracle_mod):
+    torch = torch_mod
+    # empty batch: legal, no work
+    e = torch.empty((0, 6, 6), dtype=torch.float64, device="cuda")
+    o = torch.empty(0, dtype=torch.float64, device="cuda")
+    ctx.eval_connected(e, e, o, U=1.0)
+    # zero matrix, identity, singular (rank-1) and block-diagonal (disconnected => 0) inputs
+    n = 8
+    Z = np.zeros((1, n, n))
+    I = np.eye(n)[None]
+    x = np.linspace(0.5, 1.5, n)
+    R1 = np.outer(x, x[::-1])[None]
+    blk = np.zeros((1, n, n)); blk[0, :3, :3] = 0.3 + np.eye(3); blk[0, 3:, 3:] = 0.2 + np.eye(5)
+    G = np.concatenate([Z, I, R1, blk])
+    ref_all, ref_conn = oracle_mod.eval_all_connected(G, None, U=2.0)
+    got_all = _gpu_eval(torch, ctx, G, None, 2.0, None, "all")
+    got_conn = _gpu_eval(torch, ctx, G, None, 2.0, None, "connected")
+    np.testing.assert_allclose(got_all, ref_all, rtol=1e-10, atol=1e-12 * np.abs(ref_all).max())
+    np.testing.assert_allclose(got_conn, ref_conn, rtol=1e-10, atol=1e-12 * np.abs(ref_all).max())
+    assert got_all[0] == 0.0 and got_conn[0] == 0.0                  # zero matrix
+    assert got_conn[1] == 0.0                                        # identity: only sigma = id, disconnected
+    assert abs(got_conn[3]) <= 1e-12 * abs(got_all[3])               # two blocks: no connected diagram
+    # bad arguments fail loudly
+    from paper_2501_00675_b200 import api
+    with pytest.raises(api.CosError):
+        big = torch.empty((1, 17, 17), dtype=torch.float64, device="cuda")
+        ctx.eval_connected(big, big, torch.empty(1, dtype=torch.float64, device="cuda"))
+    with api.Context() as fresh:
+        with pytest.raises(api.CosError):
+            fresh.build_G(torch.zeros((1, 2, 2), dtype=torch.int32, device="cuda"),
+                          torch.zeros((1, 2), dtype=torch.float64, device="cuda"),
+                          torch.empty((1, 2, 2), dtype=torch.float64, device="cuda"))
+
+
+def test_probes_report_plausible_peaks(ctx):
+    tf = ctx.probe_dfma_tflops()
+    bw = ctx.probe_smem_gbs()
+    print(f"DFMA probe {tf:.2f} TFLOP/s, shared-memory probe {bw:.0f} GB/s")
+    assert 10.0 < tf < 80.0
+    assert 5e3 < bw < 1e5
