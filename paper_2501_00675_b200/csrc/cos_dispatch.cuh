@@ -2,10 +2,15 @@
 #pragma once
 #include "cos_common.cuh"
 #include "cos_kernels_generic.cuh"
+#include "cos_kernels_tiled.cuh"
 
 namespace cosb {
 
 constexpr int kGenericThreads = 256;
+constexpr int kTiledB = 3;
+constexpr int kTiledThreads = 128;
+constexpr int kTiledNA = 4, kTiledJB = 5;
+constexpr int kTiledMinN = 5, kTiledMaxN = 12;
 
 inline size_t generic_smem_bytes(int n, int nsp)
 {
@@ -18,9 +23,25 @@ inline bool generic_needs_global(int n, int smem_optin)
     return generic_smem_bytes(n, 2) > (size_t)smem_optin;
 }
 
+// Configurations per CTA of the tiled kernel (0: the tiled kernel cannot run this order).
+inline int tiled_group(int n, int nsp, int smem_optin)
+{
+    if (n < kTiledMinN || n > kTiledMaxN) return 0;
+    if (tiled_smem_bytes<kTiledB>(n, 1, nsp) > (size_t)smem_optin) return 0;
+    const int q = n - kTiledB - 1;                       // widest stage
+    const int widest = kBinomHost.c[q][q / 2];
+    int G = (kTiledThreads + widest - 1) / widest;
+    const size_t budget = 112 * 1024;                    // keep two CTAs per SM where possible
+    while (G > 1 && tiled_smem_bytes<kTiledB>(n, G, nsp) > budget) --G;
+    return G;
+}
+
+inline bool uses_tiled(int n, int nsp, int smem_optin) { return tiled_group(n, nsp, smem_optin) > 0; }
+
 // Doubles of global scratch per CTA (0: everything lives in shared memory).
 inline size_t eval_scratch_doubles(int n, int smem_optin)
 {
+    if (uses_tiled(n, 2, smem_optin)) return 0;
     if (!generic_needs_global(n, smem_optin)) return 0;
     return ((size_t)2 << n) + generic_frontier_doubles(n);
 }
@@ -32,16 +53,37 @@ inline int eval_max_ctas(int n, long long batch, int num_sms, int smem_optin)
     return (int)(batch < cap ? batch : cap);
 }
 
+using TiledKernel = void (*)(EvalArgs, TiledDims);
+inline TiledKernel tiled_kernel() { return eval_tiled_kernel<kTiledB, kTiledThreads, kTiledNA, kTiledJB>; }
+
 inline cudaError_t configure_kernels(int smem_optin)
 {
-    return cudaFuncSetAttribute(eval_generic_kernel<kGenericThreads>,
-                                cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
+    cudaError_t e = cudaFuncSetAttribute(eval_generic_kernel<kGenericThreads>,
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(tiled_kernel(), cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
 }
 
 inline cudaError_t dispatch_eval(const EvalArgs& a, cudaStream_t stream, int num_sms, int smem_optin,
                                  int* launches, const char** name)
 {
     const int nsp = (a.Gdn == a.Gup) ? 1 : 2;
+    *launches = 1;
+    const int G = tiled_group(a.n, nsp, smem_optin);
+    if (G > 0) {
+        const TiledDims d = tiled_dims<kTiledB>(a.n, G, nsp);
+        const size_t smem = tiled_smem_bytes<kTiledB>(a.n, G, nsp);
+        int per_sm = 1;
+        cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, tiled_kernel(), kTiledThreads, smem);
+        if (e != cudaSuccess) return e;
+        if (per_sm < 1) per_sm = 1;
+        const long long groups = (a.batch + G - 1) / G;
+        long long grid = (long long)num_sms * per_sm;
+        if (grid > groups) grid = groups;
+        tiled_kernel()<<<(unsigned)grid, kTiledThreads, smem, stream>>>(a, d);
+        *name = "eval_tiled_kernel";
+        return cudaGetLastError();
+    }
     const bool use_global = generic_needs_global(a.n, smem_optin);
     const size_t smem = use_global ? sizeof(double) * generic_small_doubles(a.n) : generic_smem_bytes(a.n, nsp);
     int per_sm = 1;
@@ -56,7 +98,6 @@ inline cudaError_t dispatch_eval(const EvalArgs& a, cudaStream_t stream, int num
     }
     if (grid > a.batch) grid = a.batch;
     eval_generic_kernel<kGenericThreads><<<(unsigned)grid, kGenericThreads, smem, stream>>>(a, nsp, use_global ? 1 : 0);
-    *launches = 1;
     *name = "eval_generic_kernel";
     return cudaGetLastError();
 }
