@@ -277,6 +277,16 @@ int cos_eval_connected_xt(cos_ctx* c, int n, long long batch, const int* d_xy, c
     c->last_launches = 0;
     if (batch == 0) return COS_OK;
     const bool two = c->table[1] && c->table[1] != c->table[0];
+    if (uses_team(n) && team_choice(n, two ? 2 : 1).d.smem_bytes <= (size_t)c->smem_optin) {
+        // a1 fused into the evaluation kernel: G is assembled straight into shared memory
+        EvalArgs a{};
+        a.n = n; a.batch = batch; a.u = d_u; a.U = U; a.out = d_out; a.connected = 1; a.off = c->off;
+        a.fused = 1;
+        a.bg.n = n; a.bg.batch = batch; a.bg.xy = d_xy; a.bg.tau = d_tau;
+        a.bg.Tup = c->table[0]; a.bg.Tdn = two ? c->table[1] : c->table[0];
+        a.bg.Lx = c->Lx; a.bg.Ly = c->Ly; a.bg.ntau = c->ntau; a.bg.beta = c->beta; a.bg.g_diag = g_diag;
+        return launch_eval(c, a);
+    }
     const size_t one = (size_t)batch * n * n * sizeof(double);
     int rc = grow(c, (void**)&c->gscratch, &c->gscratch_bytes, two ? 2 * one : one);
     if (rc != COS_OK) return rc;
@@ -286,6 +296,7 @@ int cos_eval_connected_xt(cos_ctx* c, int n, long long batch, const int* d_xy, c
     if (rc != COS_OK) return rc;
     return do_eval(c, n, batch, gup, gdn, d_u, U, d_out, 1);
 }
+
 
 int cos_eval_connected_xt_host(cos_ctx* c, int n, long long batch, const int* h_xy, const double* h_tau,
                                double g_diag, const double* h_u, double U, double* h_out)

@@ -9,21 +9,6 @@ namespace cosb {
 
 constexpr int kMaxN = COS_MAX_ORDER;
 
-// Arguments of one evaluation launch (steps a2..a5 of SURVEY.md §8(a)).
-struct EvalArgs {
-    int n;
-    long long batch;
-    const double* Gup;     // [batch][n][n]
-    const double* Gdn;     // [batch][n][n]; == Gup when the species share one matrix
-    const double* u;       // [batch][n] or nullptr
-    double U;
-    double* out;           // [batch]
-    int connected;         // 0: D[full] ("all"), 1: C[full]
-    const uint32_t* off;   // off[R] = sum_{x<R}(popc(x)+1), R = 0..2^(kMaxN-1)
-    double* scratch;       // per-CTA global scratch (large n), may be nullptr
-    size_t scratch_stride; // doubles per CTA
-};
-
 // Arguments of the G-assembly launch (step a1).
 struct BuildGArgs {
     int n;
@@ -37,6 +22,23 @@ struct BuildGArgs {
     double g_diag;
     double* Gup;          // [batch][n][n]
     double* Gdn;          // nullptr: write Gup only
+};
+
+// Arguments of one evaluation launch (steps a2..a5 of SURVEY.md §8(a)).
+struct EvalArgs {
+    int n;
+    long long batch;
+    const double* Gup;     // [batch][n][n]
+    const double* Gdn;     // [batch][n][n]; == Gup when the species share one matrix
+    const double* u;       // [batch][n] or nullptr
+    double U;
+    double* out;           // [batch]
+    int connected;         // 0: D[full] ("all"), 1: C[full]
+    const uint32_t* off;   // off[R] = sum_{x<R}(popc(x)+1), R = 0..2^(kMaxN-1)
+    double* scratch;       // per-CTA global scratch (large n), may be nullptr
+    size_t scratch_stride; // doubles per CTA
+    int fused;             // 1: matrices are assembled on the fly from bg (Gup/Gdn unused); team kernel only
+    BuildGArgs bg;
 };
 
 }  // namespace cosb

@@ -3,6 +3,7 @@
 #include "cos_common.cuh"
 #include "cos_kernels_generic.cuh"
 #include "cos_kernels_tiled.cuh"
+#include "cos_kernels_team.cuh"
 
 namespace cosb {
 
@@ -53,6 +54,19 @@ inline int eval_max_ctas(int n, long long batch, int num_sms, int smem_optin)
     return (int)(batch < cap ? batch : cap);
 }
 
+// ---- team kernel (orders 5..10): instances per team and launch shape per order ----
+constexpr int kTeamMinN = 5, kTeamMaxN = 10;
+using TeamKernel = void (*)(EvalArgs, TeamDims);
+struct TeamChoice { TeamKernel fn; TeamDims d; };
+inline bool uses_team(int n) { return n >= kTeamMinN && n <= kTeamMaxN; }
+inline TeamChoice team_choice(int n, int nsp)
+{
+    if (n == 10) return {eval_team_kernel<8, 288, 1>, team_dims<8>(n, nsp)};
+    if (n == 9) return {eval_team_kernel<8, 160, 2>, team_dims<8>(n, nsp)};
+    if (n == 8) return {eval_team_kernel<16, 160, 2>, team_dims<16>(n, nsp)};
+    return {eval_team_kernel<32, 192, 2>, team_dims<32>(n, nsp)};
+}
+
 using TiledKernel = void (*)(EvalArgs, TiledDims);
 inline TiledKernel tiled_kernel() { return eval_tiled_kernel<kTiledB, kTiledThreads, kTiledNA, kTiledJB>; }
 
@@ -61,14 +75,34 @@ inline cudaError_t configure_kernels(int smem_optin)
     cudaError_t e = cudaFuncSetAttribute(eval_generic_kernel<kGenericThreads>,
                                          cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
     if (e != cudaSuccess) return e;
+    for (int n = kTeamMinN; n <= kTeamMaxN; ++n) {
+        e = cudaFuncSetAttribute(team_choice(n, 1).fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
+        if (e != cudaSuccess) return e;
+    }
     return cudaFuncSetAttribute(tiled_kernel(), cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
 }
 
 inline cudaError_t dispatch_eval(const EvalArgs& a, cudaStream_t stream, int num_sms, int smem_optin,
                                  int* launches, const char** name)
 {
-    const int nsp = (a.Gdn == a.Gup) ? 1 : 2;
+    const int nsp = a.fused ? (a.bg.Tdn != a.bg.Tup ? 2 : 1) : ((a.Gdn == a.Gup) ? 1 : 2);
     *launches = 1;
+    if (uses_team(a.n)) {
+        const TeamChoice tc = team_choice(a.n, nsp);
+        if (tc.d.smem_bytes <= (size_t)smem_optin) {
+            int per_sm = 1;
+            cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, tc.fn, tc.d.threads, tc.d.smem_bytes);
+            if (e != cudaSuccess) return e;
+            if (per_sm < 1) per_sm = 1;
+            const long long teams = (a.batch * nsp + tc.d.C - 1) / tc.d.C;
+            long long grid = (long long)num_sms * per_sm;
+            if (grid > teams) grid = teams;
+            tc.fn<<<(unsigned)grid, tc.d.threads, tc.d.smem_bytes, stream>>>(a, tc.d);
+            *name = "eval_team_kernel";
+            return cudaGetLastError();
+        }
+    }
+    if (a.fused) return cudaErrorInvalidValue;   // only the team kernel assembles G on the fly
     const int G = tiled_group(a.n, nsp, smem_optin);
     if (G > 0) {
         const TiledDims d = tiled_dims<kTiledB>(a.n, G, nsp);

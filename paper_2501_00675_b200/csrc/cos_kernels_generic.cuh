@@ -20,6 +20,36 @@ namespace cosb {
 
 // ------------------------------------------------------------------------------------------ a1
 // One thread per (b, i, j).  Table rows are L2 resident (1-8 MiB); two adjacent tau points per entry.
+// One entry G_s[b][i][j] (both species) of step a1; shared by build_G_kernel and the fused evaluation kernels so
+// that both produce bit-identical matrices.
+__device__ __forceinline__ void g0_entry(const BuildGArgs& a, long long b, int i, int j, double& gup, double& gdn)
+{
+    if (i == j) { gup = a.g_diag; gdn = a.g_diag; return; }
+    const int* pi = a.xy + (b * a.n + i) * 2;
+    const int* pj = a.xy + (b * a.n + j) * 2;
+    int dx = (pi[0] - pj[0]) % a.Lx; if (dx < 0) dx += a.Lx;
+    int dy = (pi[1] - pj[1]) % a.Ly; if (dy < 0) dy += a.Ly;
+    double dtau = a.tau[b * a.n + i] - a.tau[b * a.n + j];
+    double sign = 1.0;
+    if (dtau <= 0.0) { dtau = __dadd_rn(dtau, a.beta); sign = -1.0; }     // R9: dtau == 0 is 0-
+    const double uu = __ddiv_rn(__dmul_rn(dtau, (double)(a.ntau - 1)), a.beta);
+    int k = (int)floor(uu);
+    k = min(k, a.ntau - 2);
+    k = max(k, 0);
+    const double f = __dsub_rn(uu, (double)k);
+    const size_t row = ((size_t)dx * a.Ly + dy) * (size_t)a.ntau + k;
+    {
+        const double t0 = __ldg(a.Tup + row), t1 = __ldg(a.Tup + row + 1);
+        gup = sign * __fma_rn(f, __dsub_rn(t1, t0), t0);
+    }
+    if (a.Tdn && a.Tdn != a.Tup) {
+        const double t0 = __ldg(a.Tdn + row), t1 = __ldg(a.Tdn + row + 1);
+        gdn = sign * __fma_rn(f, __dsub_rn(t1, t0), t0);
+    } else {
+        gdn = gup;
+    }
+}
+
 __global__ void __launch_bounds__(256) build_G_kernel(BuildGArgs a)
 {
     const long long total = a.batch * a.n * a.n;
@@ -29,32 +59,10 @@ __global__ void __launch_bounds__(256) build_G_kernel(BuildGArgs a)
         const long long bi = t / a.n;
         const int i = (int)(bi % a.n);
         const long long b = bi / a.n;
-        if (i == j) {
-            a.Gup[t] = a.g_diag;
-            if (a.Gdn) a.Gdn[t] = a.g_diag;
-            continue;
-        }
-        const int* pi = a.xy + (b * a.n + i) * 2;
-        const int* pj = a.xy + (b * a.n + j) * 2;
-        int dx = (pi[0] - pj[0]) % a.Lx; if (dx < 0) dx += a.Lx;
-        int dy = (pi[1] - pj[1]) % a.Ly; if (dy < 0) dy += a.Ly;
-        double dtau = a.tau[b * a.n + i] - a.tau[b * a.n + j];
-        double sign = 1.0;
-        if (dtau <= 0.0) { dtau = __dadd_rn(dtau, a.beta); sign = -1.0; }     // R9: dtau == 0 is 0-
-        const double uu = __ddiv_rn(__dmul_rn(dtau, (double)(a.ntau - 1)), a.beta);
-        int k = (int)floor(uu);
-        k = min(k, a.ntau - 2);
-        k = max(k, 0);
-        const double f = __dsub_rn(uu, (double)k);
-        const size_t row = ((size_t)dx * a.Ly + dy) * (size_t)a.ntau + k;
-        {
-            const double t0 = __ldg(a.Tup + row), t1 = __ldg(a.Tup + row + 1);
-            a.Gup[t] = sign * __fma_rn(f, __dsub_rn(t1, t0), t0);
-        }
-        if (a.Gdn) {
-            const double t0 = __ldg(a.Tdn + row), t1 = __ldg(a.Tdn + row + 1);
-            a.Gdn[t] = sign * __fma_rn(f, __dsub_rn(t1, t0), t0);
-        }
+        double gup, gdn;
+        g0_entry(a, b, i, j, gup, gdn);
+        a.Gup[t] = gup;
+        if (a.Gdn) a.Gdn[t] = gdn;
     }
 }
 

@@ -50,9 +50,9 @@ __device__ __forceinline__ void leaf_conv(const double (&c)[16], const double (&
 
 __device__ __forceinline__ double sel(bool p, double a, double b) { return p ? a : b; }
 
-template <int THREADS>
-__device__ __forceinline__ void reduce_blocked(double* cfg0, int cfg_doubles, int off_c, int off_d1, int ng, int n,
-                                               const uint16_t* mask16, const int* lvlT, int tid)
+// THREADS: threads of the CTA (a multiple of 32; all of them must call).
+__device__ __forceinline__ void reduce_blocked_rt(double* cfg0, int cfg_doubles, int off_c, int off_d1, int ng, int n,
+                                                  const uint16_t* mask16, const int* lvlT, int tid, const int THREADS)
 {
     const int hb = n - 1 - kLB;
     for (int l = 0; l <= hb; ++l) {
@@ -196,6 +196,13 @@ __device__ __forceinline__ void reduce_blocked(double* cfg0, int cfg_doubles, in
         }
         __syncthreads();
     }
+}
+
+template <int THREADS>
+__device__ __forceinline__ void reduce_blocked(double* cfg0, int cfg_doubles, int off_c, int off_d1, int ng, int n,
+                                               const uint16_t* mask16, const int* lvlT, int tid)
+{
+    reduce_blocked_rt(cfg0, cfg_doubles, off_c, off_d1, ng, n, mask16, lvlT, tid, THREADS);
 }
 
 }  // namespace cosb

@@ -125,11 +125,41 @@ def test_fused_xt_and_host_paths(torch_mod, ctx, oracle_mod):
     out = torch.empty(w.batch, dtype=torch.float64, device="cuda")
     ctx.eval_connected_xt(_dev(torch, w.xy), _dev(torch, w.tau), out, U=w.U)
     torch.cuda.synchronize()
-    assert ctx.last_launch_count() >= 2
+    assert ctx.last_launch_count() >= 1
     check_parity(oracle_mod, out.cpu().numpy(), Gup, None, w.U, None, "connected")
     h_out = np.empty(w.batch)
     ctx.eval_connected_xt_host(w.xy, w.tau, h_out, U=w.U)
     np.testing.assert_array_equal(h_out, out.cpu().numpy())
+    # the fused entry assembles exactly the matrices cos_build_G writes: same value as the two-call route
+    G = torch.empty((w.batch, w.n, w.n), dtype=torch.float64, device="cuda")
+    ctx.build_G(_dev(torch, w.xy), _dev(torch, w.tau), G, None, g_diag=0.0)
+    out2 = torch.empty_like(out)
+    ctx.eval_connected(G, G, out2, U=w.U)
+    torch.cuda.synchronize()
+    np.testing.assert_array_equal(out2.cpu().numpy(), out.cpu().numpy())
+
+
+@pytest.mark.parametrize("n,B", [(5, 77), (8, 130), (10, 45), (12, 21)])
+def test_fused_xt_two_tables(torch_mod, oracle_mod, n, B):
+    """Fused entry with distinct spin-up / spin-down tables (two propagation instances per configuration),
+    per-vertex couplings and a non-zero equal-time diagonal; ragged batch sizes."""
+    torch = torch_mod
+    from paper_2501_00675_b200 import api
+    rng = np.random.default_rng(77 + n)
+    L, ntau, beta = 6, 41, 2.9
+    Tu = rng.normal(size=(L, L, ntau)) * 0.6
+    Td = rng.normal(size=(L, L, ntau)) * 0.6
+    xy = rng.integers(0, L, size=(B, n, 2)).astype(np.int32)
+    tau = rng.uniform(0, beta, size=(B, n))
+    u = rng.uniform(0.5, 1.5, size=(B, n))
+    Gup, Gdn = oracle_mod.build_G(xy, tau, Tu, Td, beta, 0.3)
+    with api.Context() as c2:
+        c2.set_g0_table(_dev(torch, Tu), beta, spin=0)
+        c2.set_g0_table(_dev(torch, Td), beta, spin=1)
+        out = torch.empty(B, dtype=torch.float64, device="cuda")
+        c2.eval_connected_xt(_dev(torch, xy), _dev(torch, tau), out, U=1.0, d_u=_dev(torch, u), g_diag=0.3)
+        torch.cuda.synchronize()
+        check_parity(oracle_mod, out.cpu().numpy(), Gup, Gdn, 1.0, u, "connected")
 
 
 def test_degenerate_inputs(torch_mod, ctx, oracle_mod):
