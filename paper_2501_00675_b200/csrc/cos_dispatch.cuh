@@ -61,7 +61,7 @@ struct TeamChoice { TeamKernel fn; TeamDims d; };
 inline bool uses_team(int n) { return n >= kTeamMinN && n <= kTeamMaxN; }
 inline TeamChoice team_choice(int n, int nsp)
 {
-    if (n == 10) return {eval_team_kernel<8, 288, 1>, team_dims<8>(n, nsp)};
+    if (n == 10) return {eval_team_kernel<4, 160, 2>, team_dims<4>(n, nsp)};
     if (n == 9) return {eval_team_kernel<8, 160, 2>, team_dims<8>(n, nsp)};
     if (n == 8) return {eval_team_kernel<16, 160, 2>, team_dims<16>(n, nsp)};
     return {eval_team_kernel<32, 192, 2>, team_dims<32>(n, nsp)};

@@ -10,7 +10,10 @@
 //        node record (S_Q, c)   : [part 0..3][instance 0..C-1][2 doubles]   (the 8 values R_T subset of T)
 //        W entry (c, c')        : [replica 0..REP-1][instance 0..C-1]        REP = 16 / C  (C < 16)
 //    The W gather is the only lane-dependent address; with REP replicas the (at most 16 / C) patterns of a
-//    half warp read different bank groups, so it is conflict free by construction as well.
+//    half warp read different bank groups, so it is conflict free by construction.  For C = 4 a quarter warp
+//    spans two patterns; the part index of a record is XOR-ed with the parity of the record number so that
+//    consecutive records (consecutive patterns read the same source position) use different halves of a
+//    128-byte row.
 //  * vertices are split into T = {0,1,2} and Q = {3..n-1} as in the tiled kernel: one thread carries the 8
 //    subsets R_T of one Q-pattern, every W entry it loads is used 8 times, transitions inside T stay in
 //    registers, and every FMA executed is one the method needs.
@@ -20,23 +23,47 @@
 //    (n-3)(n-2)/2, and a level exposes C(n-3, j+1) x C items of parallel work.
 //  * the two species of one configuration are two instances of the same team, so G_up != G_dn costs no
 //    extra shared memory per instance.
+//  * the connected reduction (step a4) runs on configuration-interleaved blocks of 16 values (the 4 lowest
+//    vertices of S' in registers), the terms of one output split over up to 32 / NC lanes of one warp.
 #pragma once
 #include "cos_common.cuh"
 #include "cos_kernels_generic.cuh"
-#include "cos_kernels_tiled.cuh"   // kBinom, cpopc, reduce_blocked_rt
+#include "cos_kernels_tiled.cuh"   // kBinom, cpopc
 
 namespace cosb {
 
 constexpr int kTeamB = 3;          // |T|
 constexpr int kTeamNT = 8;         // 2^|T|
-constexpr int kTeamMaxTargets = 6; // Q-targets held in registers per pass (orders <= 10 need at most 6)
+constexpr int kTeamMaxTargets = 6; // Q-targets held in registers (orders <= 10 need at most 6)
+constexpr int kRedLB = 4;          // low bits of S' held in registers by the reduction
 
 template <int C> struct TeamLayout {
-    static_assert(C == 8 || C == 16 || C == 32, "instances per team");
+    static_assert(C == 4 || C == 8 || C == 16 || C == 32, "instances per team");
     static constexpr int REP = (C >= 16) ? 1 : 16 / C;   // W replicas
     static constexpr int WE = REP * C;                   // doubles per W entry
     static constexpr int PART = 2 * C;                   // doubles per record part
     static constexpr int REC = 8 * C;                    // doubles per node record
+    static constexpr int SWZ = (C >= 8) ? 0 : (8 / C - 1);   // part-index swizzle mask (by record number)
+};
+
+// Pointers to the even (0, 2) and odd (1, 3) parts of record `rec`: part p lives at (p & 1 ? odd : even) + p * PART.
+template <int C>
+struct RecPtr {
+    double* even;
+    double* odd;
+    __device__ __forceinline__ RecPtr(double* base, int rec)
+    {
+        using L = TeamLayout<C>;
+        double* p = base + rec * L::REC;
+        if (L::SWZ) {
+            const int b = (rec & 1) * L::PART;
+            even = p + b;
+            odd = p - b;
+        } else {
+            even = odd = p;
+        }
+    }
+    __device__ __forceinline__ double* part(int p) const { return ((p & 1) ? odd : even) + p * TeamLayout<C>::PART; }
 };
 
 struct TeamDims {
@@ -47,8 +74,9 @@ struct TeamDims {
     int maxrec;        // records per frontier buffer
     int zrec;          // Z records (2^qmax)
     int ncfg;          // configurations per team = C / nsp
-    int red_stride;    // doubles per configuration of the reduction arrays
+    int red_rows;      // 2^(n-1-kRedLB) block rows of the reduction arrays
     int off_w, off_u, off_z, off_b0, off_b1;   // double offsets behind the tables
+    int off_cb, off_db;                        // reduction arrays (alias the frontier buffers)
     int tab_bytes;
     size_t smem_bytes;
 };
@@ -68,12 +96,12 @@ inline TeamDims team_dims(int n, int nsp)
     TeamDims d{};
     d.n = n; d.nsp = nsp; d.C = C;
     d.qmax = n - kTeamB;
-    const int lanes_pat = 32 / (C < 32 ? C : 32);         // patterns per warp
+    const int lanes_pat = 32 / C;                         // patterns per warp
     int slots = team_max_patterns(n);
     slots = (slots + lanes_pat - 1) / lanes_pat * lanes_pat;
+    if (slots * C < 64) slots = 64 / C;
     d.pslots = slots;
     d.threads = slots * C;
-    if (d.threads < 64) { d.threads = 64; d.pslots = 64 / C; }
     int maxrec = 1;
     for (int j = 0; j <= d.qmax; ++j) {
         const int v = j * kBinomHost.c[d.qmax][j + 1];
@@ -82,16 +110,18 @@ inline TeamDims team_dims(int n, int nsp)
     d.maxrec = maxrec;
     d.zrec = 1 << d.qmax;
     d.ncfg = C / nsp;
-    d.red_stride = red_doubles(n) + 2;
+    d.red_rows = 1 << (n - 1 - kRedLB);
     d.off_w = 0;
     d.off_u = d.off_w + n * n * L::WE;
-    d.off_z = d.off_u + C * 64;                           // per configuration: wlo[32], whi[32]
+    d.off_z = d.off_u + 16 * d.ncfg;                      // un[v][cfg] = -u_v
     d.off_b0 = d.off_z + d.zrec * L::REC;
     int work = 2 * maxrec * L::REC;
-    const int need = d.ncfg * d.red_stride;
+    const int need = 2 * d.red_rows * 16 * d.ncfg;
     if (work < need) work = need;
     d.off_b1 = d.off_b0 + maxrec * L::REC;
-    d.tab_bytes = ((2 * 2 * (1 << (n - 1)) + 4 * 64) + 15) & ~15;
+    d.off_cb = d.off_b0;
+    d.off_db = d.off_b0 + d.red_rows * 16 * d.ncfg;
+    d.tab_bytes = ((2 * 2 * (1 << (n - 1)) + 4 * 64 + 2 * d.zrec) + 15) & ~15;   // mask16, rank16, lvlT, lvlZ, recSQ
     d.smem_bytes = (size_t)d.tab_bytes + sizeof(double) * (size_t)(d.off_b0 + work);
     return d;
 }
@@ -105,6 +135,17 @@ struct TeamLevel {
     const uint16_t* rank16;
 };
 
+template <int C>
+__device__ __forceinline__ void team_load_rec(const RecPtr<C>& r, double (&a)[kTeamNT])
+{
+#pragma unroll
+    for (int p = 0; p < 4; ++p) {
+        const double2 v2 = *reinterpret_cast<const double2*>(r.part(p));
+        a[2 * p] = v2.x;
+        a[2 * p + 1] = v2.y;
+    }
+}
+
 // One item: Q-pattern SQ (|SQ| = j + 1, top element q, stage vertex h = q + 3) of one instance.
 //   sm : shared doubles, already offset by the instance (g * 2)
 //   Wl : W of this instance and replica, entry (c, c') at Wl[(c * n + c') * WE]
@@ -113,13 +154,13 @@ template <int C, int N>
 __device__ __forceinline__ void team_item(const TeamLevel& L, unsigned SQ, int x, double* sm, const double* Wl)
 {
     using Lay = TeamLayout<C>;
-    constexpr int WE = Lay::WE, REC = Lay::REC, PART = Lay::PART, NT = kTeamNT, B = kTeamB;
+    constexpr int WE = Lay::WE, NT = kTeamNT, B = kTeamB;
     const int n = L.n;
     const int q = 31 - __clz((int)SQ);
     const unsigned RQ = SQ ^ (1u << q);
     const int h = q + B;
     int colo[N + 1];                  // W column offset of target k; the last one is the close column h
-    int orec[N > 0 ? N : 1];          // double offset of target k's record in the next buffer
+    int orec[N > 0 ? N : 1];          // record number of target k in the next buffer
     {
         unsigned absent = ~RQ & ((1u << q) - 1u);
 #pragma unroll
@@ -127,45 +168,43 @@ __device__ __forceinline__ void team_item(const TeamLevel& L, unsigned SQ, int x
             const int d = __ffs(absent) - 1;
             absent &= absent - 1;
             colo[k] = (d + B) * WE;
-            orec[k] = (__popc(RQ & ((1u << d) - 1u)) * L.cnt_next + L.rank16[SQ | (1u << d)]) * REC;
+            orec[k] = __popc(RQ & ((1u << d) - 1u)) * L.cnt_next + L.rank16[SQ | (1u << d)];
         }
         colo[N] = h * WE;
     }
+    const int rowstride = n * WE;
     double acc[NT][N + 1], accT[NT][B];
-#pragma unroll
-    for (int t = 0; t < NT; ++t) {
-#pragma unroll
-        for (int k = 0; k <= N; ++k) acc[t][k] = 0.0;
-#pragma unroll
-        for (int tp = 0; tp < B; ++tp) accT[t][tp] = 0.0;
-    }
-    // ---- phase 1: sources in Q (streamed from the level buffer) and the start node h (from Z) ----
+    // ---- phase 1a: the start node (S, h) = Z[S \ {h}] ("top node", one per stage) ----
     {
-        const double* rec = sm + L.off_cur + x * REC;
-        const int step = L.cnt * REC;
-        const double* zsrc = sm + L.off_z + (L.lvlZ_j + L.rank16[RQ]) * REC;
+        const RecPtr<C> zp(sm + L.off_z, L.lvlZ_j + L.rank16[RQ]);
+        double a[NT];
+        team_load_rec<C>(zp, a);
+        const double* row = Wl + h * rowstride;
+#pragma unroll
+        for (int k = 0; k <= N; ++k) {
+            const double w = row[colo[k]];
+#pragma unroll
+            for (int t = 0; t < NT; ++t) acc[t][k] = a[t] * w;
+        }
+#pragma unroll
+        for (int tp = 0; tp < B; ++tp) {
+            const double w = row[tp * WE];
+#pragma unroll
+            for (int t = 0; t < NT; ++t) accT[t][tp] = ((t >> tp) & 1) ? 0.0 : a[t] * w;
+        }
+    }
+    // ---- phase 1b: sources in Q, streamed from the level buffer ----
+    {
         unsigned m = RQ;
-        const int rowstride = n * WE;
-        for (int i = 0; i <= L.j; ++i) {
-            const double* p;
-            int v;
-            if (i < L.j) {
-                v = __ffs(m) - 1 + B;
-                m &= m - 1;
-                p = rec;
-                rec += step;
-            } else {
-                v = h;
-                p = zsrc;
-            }
+        int rec = x;
+        for (int i = 0; i < L.j; ++i) {
+            const int v = __ffs(m) - 1 + B;
+            m &= m - 1;
+            const RecPtr<C> rp(sm + L.off_cur, rec);
+            rec += L.cnt;
             const double* row = Wl + v * rowstride;
             double a[NT];
-#pragma unroll
-            for (int t = 0; t < NT; t += 2) {
-                const double2 v2 = *reinterpret_cast<const double2*>(p + (t >> 1) * PART);
-                a[t] = v2.x;
-                a[t + 1] = v2.y;
-            }
+            team_load_rec<C>(rp, a);
 #pragma unroll
             for (int k = 0; k <= N; ++k) {
                 const double w = row[colo[k]];
@@ -201,7 +240,7 @@ __device__ __forceinline__ void team_item(const TeamLevel& L, unsigned SQ, int x
     for (int k = 0; k <= N; ++k)
 #pragma unroll
         for (int ts = 0; ts < B; ++ts) {
-            const double w = Wl[ts * n * WE + colo[k]];
+            const double w = Wl[ts * rowstride + colo[k]];
 #pragma unroll
             for (int t = 0; t < NT; ++t)
                 if ((t >> ts) & 1) acc[t][k] = fma(accT[t ^ (1 << ts)][ts], w, acc[t][k]);
@@ -209,16 +248,31 @@ __device__ __forceinline__ void team_item(const TeamLevel& L, unsigned SQ, int x
     // ---- outputs: next-level records, and Z[(SQ, R_T)] = -close (one -1 per closed fermion loop) ----
 #pragma unroll
     for (int k = 0; k < N; ++k) {
-        double* o = sm + L.off_nxt + orec[k];
+        const RecPtr<C> o(sm + L.off_nxt, orec[k]);
 #pragma unroll
-        for (int t = 0; t < NT; t += 2)
-            *reinterpret_cast<double2*>(o + (t >> 1) * PART) = make_double2(acc[t][k], acc[t + 1][k]);
+        for (int p = 0; p < 4; ++p)
+            *reinterpret_cast<double2*>(o.part(p)) = make_double2(acc[2 * p][k], acc[2 * p + 1][k]);
     }
     {
-        double* o = sm + L.off_z + (L.lvlZ_j1 + x) * REC;
+        const RecPtr<C> o(sm + L.off_z, L.lvlZ_j1 + x);
 #pragma unroll
-        for (int t = 0; t < NT; t += 2)
-            *reinterpret_cast<double2*>(o + (t >> 1) * PART) = make_double2(-acc[t][N], -acc[t + 1][N]);
+        for (int p = 0; p < 4; ++p)
+            *reinterpret_cast<double2*>(o.part(p)) = make_double2(-acc[2 * p][N], -acc[2 * p + 1][N]);
+    }
+}
+
+template <int C>
+__device__ __forceinline__ void team_dispatch_item(const TeamLevel& L, unsigned SQ, int x, double* sm, const double* Wl)
+{
+    const int N = (31 - __clz((int)SQ)) - L.j;
+    switch (N) {
+        case 0: team_item<C, 0>(L, SQ, x, sm, Wl); break;
+        case 1: team_item<C, 1>(L, SQ, x, sm, Wl); break;
+        case 2: team_item<C, 2>(L, SQ, x, sm, Wl); break;
+        case 3: team_item<C, 3>(L, SQ, x, sm, Wl); break;
+        case 4: team_item<C, 4>(L, SQ, x, sm, Wl); break;
+        case 5: team_item<C, 5>(L, SQ, x, sm, Wl); break;
+        default: team_item<C, 6>(L, SQ, x, sm, Wl); break;
     }
 }
 
@@ -245,21 +299,229 @@ __device__ __forceinline__ void team_small_stages(const double* Wl, int n, doubl
     const double p01_0 = fma(w21, w10, z[2] * w20);       // node ({0,1}, 0) from R = {1}
     z[7] = -fma(p01_0, w02, fma(p01_1, w12, z[3] * w22)); // R = {0,1}
 #pragma unroll
-    for (int t = 0; t < 8; t += 2) *reinterpret_cast<double2*>(zr + (t >> 1) * PART) = make_double2(z[t], z[t + 1]);
+    for (int t = 0; t < 8; t += 2) *reinterpret_cast<double2*>(zr + (t >> 1) * PART) = make_double2(z[t], z[t + 1]);   // record 0: no swizzle
 }
 
-template <int C>
-__device__ __forceinline__ void team_dispatch_item(const TeamLevel& L, unsigned SQ, int x, double* sm, const double* Wl)
+// ------------------------------------------------------------------------------------------ a4
+// Connected reduction on configuration-interleaved blocks (reading R5; paper's Ref. [9]):
+//   C'[S'] = D0[S'] - sum_{T' proper subset of S'} C'[T'] * D1[S' \ T'],   S' subset of vertices 1..n-1,
+//   D0[S'] = D[S' + {0}] (array CB, becomes C' in place), D1[U] = D[U] (array DB).
+// S' = (hi, lo), lo = the 4 lowest bits.  Row hi of an array holds the 16 lo-values of every configuration:
+//   [part 0..7][configuration 0..NC-1][2 doubles], the part index XOR-ed with a fold of hi when a quarter warp
+//   spans several rows (NC < 8).  A leaf multiplies block C'[T_hi] with block D1[S_hi \ T_hi] as a subset
+//   convolution over lo (81 FMAs on 32 loaded values).  The 2^|S_hi| terms of one output are split over 2^s
+//   lanes of one warp (lane bit k owns the k-th lowest vertex of S_hi), partial blocks are summed by a
+//   recursive-halving shuffle exchange, and the diagonal block (T_hi = S_hi) is solved in registers.
+template <int NC> struct RedLayout {
+    static constexpr int ROW = 16 * NC;
+    static constexpr int PSTR = 2 * NC;
+    static constexpr int MASK = (NC >= 8) ? 0 : (8 / NC - 1);
+    static constexpr int SMAX = (NC >= 32) ? 0 : (NC == 16 ? 1 : (NC == 8 ? 2 : (NC == 4 ? 3 : 4)));
+};
+
+template <int NC>
+__device__ __forceinline__ int red_swz(unsigned hi)
 {
-    const int N = (31 - __clz((int)SQ)) - L.j;
-    switch (N) {
-        case 0: team_item<C, 0>(L, SQ, x, sm, Wl); break;
-        case 1: team_item<C, 1>(L, SQ, x, sm, Wl); break;
-        case 2: team_item<C, 2>(L, SQ, x, sm, Wl); break;
-        case 3: team_item<C, 3>(L, SQ, x, sm, Wl); break;
-        case 4: team_item<C, 4>(L, SQ, x, sm, Wl); break;
-        case 5: team_item<C, 5>(L, SQ, x, sm, Wl); break;
-        default: team_item<C, 6>(L, SQ, x, sm, Wl); break;
+    if (RedLayout<NC>::MASK == 0) return 0;
+    return (int)((__popc(hi) & 1) | ((hi ^ (hi >> 2) ^ (hi >> 4)) & 2u)) & RedLayout<NC>::MASK;
+}
+
+// element lo of configuration cg in row hi (double offset relative to the array)
+template <int NC>
+__device__ __forceinline__ int red_elem(unsigned hi, unsigned lo, int cg)
+{
+    using R = RedLayout<NC>;
+    return (int)hi * R::ROW + (int)((lo >> 1) ^ (unsigned)red_swz<NC>(hi)) * R::PSTR + cg * 2 + (int)(lo & 1u);
+}
+
+template <int NC>
+__device__ __forceinline__ void red_load_block(const double* arr, unsigned hi, int cg, double (&v)[16])
+{
+    using R = RedLayout<NC>;
+    const double* row = arr + (int)hi * R::ROW + cg * 2;
+    const int sw = red_swz<NC>(hi);
+#pragma unroll
+    for (int p = 0; p < 8; ++p) {
+        const double2 x = *reinterpret_cast<const double2*>(row + (p ^ sw) * R::PSTR);
+        v[2 * p] = x.x;
+        v[2 * p + 1] = x.y;
+    }
+}
+
+template <int NC>
+__device__ __forceinline__ void team_reduce(double* CB, const double* DB, int ncfg, int n, const uint16_t* mask16,
+                                            const int* lvlT, int tid, int nthreads)
+{
+    using R = RedLayout<NC>;
+    const int hb = n - 1 - kRedLB;
+    const int cg = tid % NC, slot = tid / NC, slots = nthreads / NC;
+    for (int l = 0; l <= hb; ++l) {
+        const int outputs = kBinom.c[hb][l];
+        int s = l < R::SMAX ? l : R::SMAX;
+        while (s > 0 && (outputs << s) > slots) --s;
+        const int per_pass = slots >> s;
+        const unsigned c = (unsigned)slot & ((1u << s) - 1u);
+        for (int base = 0; base < outputs; base += per_pass) {
+            const int o = base + (slot >> s);
+            const bool active = (o < outputs) && (cg < ncfg) && ((slot >> s) < per_pass);
+            double acc[16];
+#pragma unroll
+            for (int t = 0; t < 16; ++t) acc[t] = 0.0;
+            unsigned S = 0;
+            if (active) {
+                S = mask16[lvlT[l] + o];
+                unsigned tl = 0, m = S;
+                for (int k = 0; k < s; ++k) {            // lane bit k owns the k-th lowest vertex of S
+                    const unsigned bit = m & (0u - m);
+                    m ^= bit;
+                    if ((c >> k) & 1u) tl |= bit;
+                }
+                const unsigned rest = m;
+                unsigned Th = rest;
+                while (true) {
+                    const unsigned T = Th | tl;
+                    if (T != S) {
+                        double cb[16], db[16];
+                        red_load_block<NC>(CB, T, cg, cb);
+                        red_load_block<NC>(DB, S ^ T, cg, db);
+                        leaf_conv(cb, db, acc);
+                    }
+                    if (Th == 0) break;
+                    Th = (Th - 1) & rest;
+                }
+            }
+            // ---- sum the 2^s partial blocks: recursive halving, lane bit k keeps lo-bit k == its own bit ----
+            double* blk = CB;     // element lo at blk[red_elem(S, lo, cg)]
+            if (s == 0) {
+                if (active) {
+#pragma unroll
+                    for (int t = 0; t < 16; ++t) acc[t] = blk[red_elem<NC>(S, t, cg)] - acc[t];
+                }
+            } else {
+                double r8[8];
+                const bool b0 = c & 1u;
+#pragma unroll
+                for (int i = 0; i < 8; ++i) {
+                    const double keep = sel(b0, acc[2 * i + 1], acc[2 * i]);
+                    const double send = sel(b0, acc[2 * i], acc[2 * i + 1]);
+                    r8[i] = keep + __shfl_xor_sync(0xffffffffu, send, NC);
+                }
+                if (s == 1) {
+                    if (active) {
+#pragma unroll
+                        for (int i = 0; i < 8; ++i) { const int e = red_elem<NC>(S, 2 * i + (int)b0, cg); blk[e] = blk[e] - r8[i]; }
+                    }
+                } else {
+                    double r4[4];
+                    const bool b1 = (c >> 1) & 1u;
+#pragma unroll
+                    for (int i = 0; i < 4; ++i) {
+                        const double keep = sel(b1, r8[2 * i + 1], r8[2 * i]);
+                        const double send = sel(b1, r8[2 * i], r8[2 * i + 1]);
+                        r4[i] = keep + __shfl_xor_sync(0xffffffffu, send, (NC * 2) & 31);
+                    }
+                    if (s == 2) {
+                        if (active) {
+#pragma unroll
+                            for (int i = 0; i < 4; ++i) { const int e = red_elem<NC>(S, 4 * i + (int)(c & 3u), cg); blk[e] = blk[e] - r4[i]; }
+                        }
+                    } else {
+                        double r2[2];
+                        const bool b2 = (c >> 2) & 1u;
+#pragma unroll
+                        for (int i = 0; i < 2; ++i) {
+                            const double keep = sel(b2, r4[2 * i + 1], r4[2 * i]);
+                            const double send = sel(b2, r4[2 * i], r4[2 * i + 1]);
+                            r2[i] = keep + __shfl_xor_sync(0xffffffffu, send, (NC * 4) & 31);
+                        }
+                        if (s == 3) {
+                            if (active) {
+#pragma unroll
+                                for (int i = 0; i < 2; ++i) { const int e = red_elem<NC>(S, 8 * i + (int)(c & 7u), cg); blk[e] = blk[e] - r2[i]; }
+                            }
+                        } else {
+                            const bool b3 = (c >> 3) & 1u;
+                            const double keep = sel(b3, r2[1], r2[0]);
+                            const double send = sel(b3, r2[0], r2[1]);
+                            const double r1 = keep + __shfl_xor_sync(0xffffffffu, send, (NC * 8) & 31);
+                            if (active) { const int e = red_elem<NC>(S, c & 15u, cg); blk[e] = blk[e] - r1; }
+                        }
+                    }
+                }
+                __syncwarp();
+                if (active && c == 0) red_load_block<NC>(CB, S, cg, acc);
+            }
+            // ---- diagonal block: x[lo] = pre[lo] - sum_{T proper subset of lo} x[T] e[lo ^ T], e = D1[hi = {}] ----
+            if (active && c == 0) {
+                double e[16];
+                red_load_block<NC>(DB, 0u, cg, e);
+#pragma unroll
+                for (int lo = 1; lo < 16; ++lo) {
+                    double v = acc[lo];
+#pragma unroll
+                    for (int T = 0; T < 16; ++T)
+                        if ((T & ~lo) == 0 && T != lo) v = fma(-acc[T], e[lo ^ T], v);
+                    acc[lo] = v;
+                }
+                double* row = CB + (int)S * R::ROW + cg * 2;
+                const int sw = red_swz<NC>(S);
+#pragma unroll
+                for (int p = 0; p < 8; ++p)
+                    *reinterpret_cast<double2*>(row + (p ^ sw) * R::PSTR) = make_double2(acc[2 * p], acc[2 * p + 1]);
+            }
+        }
+        __syncthreads();
+    }
+}
+
+// a3: D[S] = w(S) Zup[S] Zdn[S] for the NC configurations of the team, written straight into the reduction
+// arrays: S odd -> CB (D0[S >> 1]), S even -> DB (D1[S >> 1]).  One thread per (Z record, configuration): the 8
+// values R_T of record S_Q are the lo-values (S_Q & 3) * 4 + {0..3} of row hi = S_Q >> 2 in both arrays.
+// un[v * NC + cg] = -u_v of configuration cg (aliased species only; otherwise -u is folded into W).
+template <int C, int NC>
+__device__ __forceinline__ void team_combine(double* smd, const TeamDims& d, int ncfg, const uint16_t* recSQ,
+                                             int tid, int nthreads)
+{
+    using Lay = TeamLayout<C>;
+    using R = RedLayout<NC>;
+    constexpr int NSP = C / NC;
+    double* CB = smd + d.off_cb;
+    double* DB = smd + d.off_db;
+    const double* un = smd + d.off_u;
+    const int cg = tid % NC;
+    if (cg >= ncfg) return;
+    double wT[8];
+#pragma unroll
+    for (int t = 0; t < 8; ++t) wT[t] = 1.0;
+    if (NSP == 1) {
+        const double u0 = un[0 * NC + cg], u1 = un[1 * NC + cg], u2 = un[2 * NC + cg];
+#pragma unroll
+        for (int t = 0; t < 8; ++t) wT[t] = ((t & 1) ? u0 : 1.0) * ((t & 2) ? u1 : 1.0) * ((t & 4) ? u2 : 1.0);
+    }
+    for (int rec = tid / NC; rec < d.zrec; rec += nthreads / NC) {
+        const unsigned SQ = recSQ[rec];
+        double wq = 1.0;
+        if (NSP == 1) {
+            unsigned m = SQ;
+            while (m) { const int v = __ffs(m) - 1; m &= m - 1; wq *= un[(v + kTeamB) * NC + cg]; }
+        }
+        const RecPtr<C> zp(smd + d.off_z + (cg * NSP) * 2, rec);
+        double val[8];
+#pragma unroll
+        for (int p = 0; p < 4; ++p) {
+            const double2 zu = *reinterpret_cast<const double2*>(zp.part(p));
+            const double2 zd = *reinterpret_cast<const double2*>(zp.part(p) + (NSP - 1) * 2);
+            val[2 * p] = (wq * wT[2 * p]) * (zu.x * zd.x);
+            val[2 * p + 1] = (wq * wT[2 * p + 1]) * (zu.y * zd.y);
+        }
+        const unsigned hi = SQ >> 2;
+        const int pa = (int)(SQ & 3u) * 2, sw = red_swz<NC>(hi);
+        double* crow = CB + (int)hi * R::ROW + cg * 2;
+        double* drow = DB + (int)hi * R::ROW + cg * 2;
+        *reinterpret_cast<double2*>(crow + ((pa) ^ sw) * R::PSTR) = make_double2(val[1], val[3]);
+        *reinterpret_cast<double2*>(crow + ((pa + 1) ^ sw) * R::PSTR) = make_double2(val[5], val[7]);
+        *reinterpret_cast<double2*>(drow + ((pa) ^ sw) * R::PSTR) = make_double2(val[0], val[2]);
+        *reinterpret_cast<double2*>(drow + ((pa + 1) ^ sw) * R::PSTR) = make_double2(val[4], val[6]);
     }
 }
 
@@ -267,12 +529,13 @@ template <int C, int MAXT, int MINB>
 __global__ void __launch_bounds__(MAXT, MINB) eval_team_kernel(EvalArgs a, TeamDims d)
 {
     using Lay = TeamLayout<C>;
-    constexpr int WE = Lay::WE, REC = Lay::REC, PART = Lay::PART, REP = Lay::REP, B = kTeamB;
+    constexpr int WE = Lay::WE, REC = Lay::REC, PART = Lay::PART, REP = Lay::REP;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     uint16_t* mask16 = reinterpret_cast<uint16_t*>(smem_raw);
     uint16_t* rank16 = mask16 + (1 << (d.n - 1));
     int* lvlT = reinterpret_cast<int*>(rank16 + (1 << (d.n - 1)));   // list offsets, ground set n-1 bits
     int* lvlZ = lvlT + 32;                                           // Z record offsets, ground set qmax bits
+    uint16_t* recSQ = reinterpret_cast<uint16_t*>(lvlZ + 32);        // Z record -> S_Q
     double* smd = reinterpret_cast<double*>(smem_raw + d.tab_bytes);
     const int tid = threadIdx.x, nthreads = blockDim.x;
     const int n = d.n, qmax = d.qmax, nsp = d.nsp;
@@ -297,6 +560,7 @@ __global__ void __launch_bounds__(MAXT, MINB) eval_team_kernel(EvalArgs a, TeamD
         while (m) { const int s = __ffs(m) - 1; m &= m - 1; ++i; rk += kBinom.c[s][i]; }
         rank16[mk] = (uint16_t)rk;
         mask16[lvlT[i] + rk] = (uint16_t)mk;
+        if (mk < (1u << qmax)) recSQ[lvlZ[i] + rk] = (uint16_t)mk;
     }
     __syncthreads();
 
@@ -306,6 +570,7 @@ __global__ void __launch_bounds__(MAXT, MINB) eval_team_kernel(EvalArgs a, TeamD
         const long long inst0 = team * C;
         const int ninst = (int)min((long long)C, total_inst - inst0);
         const int ncfg = ninst / nsp;
+        const int NCt = C / nsp;                 // configuration slots of a team
         const long long cfgbase = inst0 / nsp;
         __syncthreads();
         // ---- a1 (fused) / load: W of every instance, instance fastest; -u_a folded into the rows of species 0
@@ -329,18 +594,11 @@ __global__ void __launch_bounds__(MAXT, MINB) eval_team_kernel(EvalArgs a, TeamD
 #pragma unroll
             for (int r = 0; r < REP; ++r) w[((r + e) % REP) * C] = val;
         }
-        // w(S) = prod_{v in S} (-u_v) as wlo[S & 31] * whi[S >> 5] (aliased species only)
+        // un[v][cfg] = -u_v (aliased species only: w(S) is applied in the combine step)
         if (nsp == 1) {
-            for (int t = tid; t < ncfg * 64; t += nthreads) {
-                const int cg = t >> 6, idx = t & 63, hi = idx >> 5;
-                unsigned bits = (unsigned)(idx & 31);
-                double w = 1.0;
-                while (bits) {
-                    const int v = __ffs(bits) - 1 + 5 * hi;
-                    bits &= bits - 1;
-                    if (v < n) w *= -(a.u ? a.u[(cfgbase + cg) * n + v] : a.U);
-                }
-                smd[d.off_u + cg * 64 + idx] = w;
+            for (int t = tid; t < NCt * n; t += nthreads) {
+                const int cg = t % NCt, v = t / NCt;
+                smd[d.off_u + v * NCt + cg] = (cg < ncfg) ? -(a.u ? a.u[(cfgbase + cg) * n + v] : a.U) : 0.0;
             }
         }
         __syncthreads();
@@ -367,35 +625,32 @@ __global__ void __launch_bounds__(MAXT, MINB) eval_team_kernel(EvalArgs a, TeamD
         // ---- a3 + a5 ("all"): D[full] = w * Zup[full] * Zdn[full] ----
         if (!a.connected) {
             if (tid < ncfg) {
-                const int full = lvlZ[qmax] * REC + 3 * PART + 1;      // S_Q = Q, R_T = T
-                const double zu = smd[d.off_z + full + (tid * nsp) * 2];
-                const double zd = smd[d.off_z + full + (tid * nsp + nsp - 1) * 2];
+                const int rec = lvlZ[qmax];                            // S_Q = Q, R_T = T: part 3, second value
+                const int part = Lay::SWZ ? (3 ^ (rec & 1)) : 3;
+                const double* zp = smd + d.off_z + rec * REC + part * PART + 1;
+                const double zu = zp[(tid * nsp) * 2];
+                const double zd = zp[(tid * nsp + nsp - 1) * 2];
                 double w = 1.0;
-                if (nsp == 1) w = smd[d.off_u + tid * 64 + ((NS - 1) & 31)] * smd[d.off_u + tid * 64 + 32 + ((NS - 1) >> 5)];
+                if (nsp == 1) for (int v = 0; v < n; ++v) w *= smd[d.off_u + v * NCt + tid];
                 a.out[cfgbase + tid] = w * zu * zd;
             }
             continue;
         }
 
-        // ---- a3: D[S] = w(S) Zup[S] Zdn[S], split by vertex 0 into D0[S'] = D[2S'+1] (becomes C' in place)
-        //      and D1[U] = D[2U], both in the padded block layout of cos_reduce_blocked.cuh ----
-        double* red = smd + d.off_b0;
-        const int off_c = 0, off_d1 = red_rows(n) * kRowStride;
-        for (unsigned t = tid; t < (unsigned)ncfg * NS; t += nthreads) {
-            const unsigned cg = t % (unsigned)ncfg, S = t / (unsigned)ncfg;
-            const unsigned SQ = S >> B, ST = S & 7u;
-            const int at = d.off_z + (lvlZ[__popc(SQ)] + rank16[SQ]) * REC + (int)(ST >> 1) * PART + (int)(ST & 1u);
-            const double zu = smd[at + (cg * nsp) * 2];
-            const double zd = smd[at + (cg * nsp + nsp - 1) * 2];
-            double w = 1.0;
-            if (nsp == 1) w = smd[d.off_u + cg * 64 + (S & 31u)] * smd[d.off_u + cg * 64 + 32 + (S >> 5)];
-            red[cg * d.red_stride + ((S & 1u) ? off_c : off_d1) + red_addr(S >> 1)] = w * zu * zd;
+        // ---- a3: combine, a4: connected reduction, a5: C'[full] ----
+        double* CB = smd + d.off_cb;
+        const double* DB = smd + d.off_db;
+        if (nsp == 1) {
+            team_combine<C, C>(smd, d, ncfg, recSQ, tid, nthreads);
+            __syncthreads();
+            team_reduce<C>(CB, DB, ncfg, n, mask16, lvlT, tid, nthreads);
+            if (tid < ncfg) a.out[cfgbase + tid] = CB[red_elem<C>((NS >> (1 + kRedLB)) - 1, 15u, tid)];
+        } else {
+            team_combine<C, C / 2>(smd, d, ncfg, recSQ, tid, nthreads);
+            __syncthreads();
+            team_reduce<C / 2>(CB, DB, ncfg, n, mask16, lvlT, tid, nthreads);
+            if (tid < ncfg) a.out[cfgbase + tid] = CB[red_elem<C / 2>((NS >> (1 + kRedLB)) - 1, 15u, tid)];
         }
-        __syncthreads();
-
-        // ---- a4: connected reduction, a5: C'[full] ----
-        reduce_blocked_rt(red, d.red_stride, off_c, off_d1, ncfg, n, mask16, lvlT, tid, nthreads);
-        if (tid < ncfg) a.out[cfgbase + tid] = red[tid * d.red_stride + off_c + red_addr((NS >> 1) - 1)];
     }
 }
 
