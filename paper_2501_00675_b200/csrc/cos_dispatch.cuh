@@ -39,9 +39,21 @@ inline int tiled_group(int n, int nsp, int smem_optin)
 
 inline bool uses_tiled(int n, int nsp, int smem_optin) { return tiled_group(n, nsp, smem_optin) > 0; }
 
+// Orders 13..16: the tiled kernel with one configuration per CTA whose block (W, Z, level buffers, reduction
+// arrays) lives in global scratch (L2 resident); only the subset tables stay in shared memory.
+constexpr int kBigThreads = 256, kBigNA = 6, kBigJB = 7, kBigMinN = 13;
+inline bool uses_big(int n) { return n >= kBigMinN && n <= kMaxN; }
+inline TiledDims big_dims(int n, int nsp)
+{
+    TiledDims d = tiled_dims<kTiledB>(n, 1, nsp);
+    d.use_global = 1;
+    return d;
+}
+
 // Doubles of global scratch per CTA (0: everything lives in shared memory).
 inline size_t eval_scratch_doubles(int n, int smem_optin)
 {
+    if (uses_big(n)) return (size_t)big_dims(n, 2).cfg_doubles;
     if (uses_tiled(n, 2, smem_optin)) return 0;
     if (!generic_needs_global(n, smem_optin)) return 0;
     return ((size_t)2 << n) + generic_frontier_doubles(n);
@@ -68,7 +80,8 @@ inline TeamChoice team_choice(int n, int nsp)
 }
 
 using TiledKernel = void (*)(EvalArgs, TiledDims);
-inline TiledKernel tiled_kernel() { return eval_tiled_kernel<kTiledB, kTiledThreads, kTiledNA, kTiledJB>; }
+inline TiledKernel tiled_kernel() { return eval_tiled_kernel<kTiledB, kTiledThreads, kTiledNA, kTiledJB, false>; }
+inline TiledKernel big_kernel() { return eval_tiled_kernel<kTiledB, kBigThreads, kBigNA, kBigJB, true>; }
 
 inline cudaError_t configure_kernels(int smem_optin)
 {
@@ -79,6 +92,8 @@ inline cudaError_t configure_kernels(int smem_optin)
         e = cudaFuncSetAttribute(team_choice(n, 1).fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
         if (e != cudaSuccess) return e;
     }
+    e = cudaFuncSetAttribute(big_kernel(), cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
+    if (e != cudaSuccess) return e;
     return cudaFuncSetAttribute(tiled_kernel(), cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
 }
 
@@ -103,6 +118,20 @@ inline cudaError_t dispatch_eval(const EvalArgs& a, cudaStream_t stream, int num
         }
     }
     if (a.fused) return cudaErrorInvalidValue;   // only the team kernel assembles G on the fly
+    if (uses_big(a.n)) {
+        const TiledDims d = big_dims(a.n, nsp);
+        const size_t smem = (size_t)d.tab_bytes;
+        int per_sm = 1;
+        cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, big_kernel(), kBigThreads, smem);
+        if (e != cudaSuccess) return e;
+        if (per_sm < 1) per_sm = 1;
+        long long grid = (long long)num_sms * per_sm;
+        const long long cap = eval_max_ctas(a.n, a.batch, num_sms, smem_optin);
+        if (grid > cap) grid = cap;
+        big_kernel()<<<(unsigned)grid, kBigThreads, smem, stream>>>(a, d);
+        *name = "eval_tiled_kernel(global)";
+        return cudaGetLastError();
+    }
     const int G = tiled_group(a.n, nsp, smem_optin);
     if (G > 0) {
         const TiledDims d = tiled_dims<kTiledB>(a.n, G, nsp);

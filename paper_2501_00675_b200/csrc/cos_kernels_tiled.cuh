@@ -65,6 +65,7 @@ struct TiledDims {
     int bufrec;      // records per level buffer
     int cfg_doubles; // doubles per configuration
     int tab_bytes;   // table bytes at the start of shared memory
+    int use_global;  // 1: the configuration block (W, Z, level buffers, reduction arrays) lives in EvalArgs::scratch
 };
 
 template <int B>
@@ -90,7 +91,7 @@ template <int B>
 inline size_t tiled_smem_bytes(int n, int G, int nsp)
 {
     const TiledDims d = tiled_dims<B>(n, G, nsp);
-    return (size_t)d.tab_bytes + sizeof(double) * (size_t)d.cfg_doubles * G;
+    return (size_t)d.tab_bytes + sizeof(double) * (size_t)d.cfg_doubles * G;   // all-in-shared-memory variant
 }
 
 // Everything an item routine needs that is uniform over the CTA for one level step.
@@ -349,7 +350,8 @@ __device__ __forceinline__ void run_level(const LevelCtx& c, int ng, int tid, in
                 case 2: item_mode_A<B, 2>(c, g, r); break;
                 case 3: item_mode_A<B, 3>(c, g, r); break;
                 case 4: item_mode_A<B, 4>(c, g, r); break;
-                default: if constexpr (NA_MAX >= 5) { item_mode_A<B, 5>(c, g, r); } break;
+                case 5: if constexpr (NA_MAX >= 5) { item_mode_A<B, 5>(c, g, r); } break;
+                default: if constexpr (NA_MAX >= 6) { item_mode_A<B, 6>(c, g, r); } break;
             }
         } else {
             switch (J1) {
@@ -358,7 +360,8 @@ __device__ __forceinline__ void run_level(const LevelCtx& c, int ng, int tid, in
                 case 3: item_mode_B<B, 3>(c, g, r); break;
                 case 4: item_mode_B<B, 4>(c, g, r); break;
                 case 5: item_mode_B<B, 5>(c, g, r); break;
-                default: if constexpr (JB_MAX >= 6) { item_mode_B<B, 6>(c, g, r); } break;
+                case 6: if constexpr (JB_MAX >= 6) { item_mode_B<B, 6>(c, g, r); } break;
+                default: if constexpr (JB_MAX >= 7) { item_mode_B<B, 7>(c, g, r); } break;
             }
         }
     }
@@ -407,7 +410,7 @@ __device__ unsigned long long g_phase_cycles[8];
 #define COS_PHASE_MARK(k) do { } while (0)
 #endif
 
-template <int B, int THREADS, int NA_MAX, int JB_MAX>
+template <int B, int THREADS, int NA_MAX, int JB_MAX, bool GLOBAL>
 __global__ void __launch_bounds__(THREADS) eval_tiled_kernel(EvalArgs a, TiledDims d)
 {
 #ifdef COS_PHASE_TIMING
@@ -420,7 +423,8 @@ __global__ void __launch_bounds__(THREADS) eval_tiled_kernel(EvalArgs a, TiledDi
     uint16_t* rank16 = mask16 + (1 << (d.n - 1));
     int* lvlT = reinterpret_cast<int*>(rank16 + (1 << (d.n - 1)));   // list offsets, ground set n-1 bits
     int* lvl = lvlT + 32;                                            // Zr record offsets, ground set qmax bits
-    double* cfg0 = reinterpret_cast<double*>(smem_raw + d.tab_bytes);
+    double* cfg0 = GLOBAL ? a.scratch + (size_t)blockIdx.x * a.scratch_stride
+                          : reinterpret_cast<double*>(smem_raw + d.tab_bytes);
     const int tid = threadIdx.x;
     const int n = d.n, qmax = d.qmax, nsp = d.nsp;
     const unsigned N = 1u << n;
