@@ -382,3 +382,17 @@ long long cos_flop_count(int n, int n_species, int connected)
 }
 
 }  // extern "C"
+
+#ifdef COS_PHASE_TIMING
+// Development aid (not part of include/cos.h; compiled only with -DCOS_PHASE_TIMING): cycles thread 0 of every
+// CTA spent in each phase of the evaluation kernels, summed over CTAs.
+extern "C" int cos_debug_phase_cycles(unsigned long long* h_out8, int reset)
+{
+    if (h_out8 && cudaMemcpyFromSymbol(h_out8, cosb::g_phase_cycles, 8 * sizeof(unsigned long long)) != cudaSuccess) return COS_ECUDA;
+    if (reset) {
+        unsigned long long z[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+        if (cudaMemcpyToSymbol(cosb::g_phase_cycles, z, sizeof(z)) != cudaSuccess) return COS_ECUDA;
+    }
+    return COS_OK;
+}
+#endif

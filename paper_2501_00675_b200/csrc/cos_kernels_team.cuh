@@ -150,6 +150,8 @@ __device__ __forceinline__ void team_load_rec(const RecPtr<C>& r, double (&a)[kT
 //   sm : shared doubles, already offset by the instance (g * 2)
 //   Wl : W of this instance and replica, entry (c, c') at Wl[(c * n + c') * WE]
 // N = q - j Q-targets are accumulated in registers together with the close (column h) and the T-targets.
+// N is the number of Q-targets of the widest item of the WARP (warp-uniform, so the dispatch never diverges); an
+// item with fewer targets (Nown < N) pads with dummy targets that read a valid W column and are never stored.
 template <int C, int N>
 __device__ __forceinline__ void team_item(const TeamLevel& L, unsigned SQ, int x, double* sm, const double* Wl)
 {
@@ -165,10 +167,15 @@ __device__ __forceinline__ void team_item(const TeamLevel& L, unsigned SQ, int x
         unsigned absent = ~RQ & ((1u << q) - 1u);
 #pragma unroll
         for (int k = 0; k < N; ++k) {
-            const int d = __ffs(absent) - 1;
-            absent &= absent - 1;
-            colo[k] = (d + B) * WE;
-            orec[k] = __popc(RQ & ((1u << d) - 1u)) * L.cnt_next + L.rank16[SQ | (1u << d)];
+            if (absent) {
+                const int d = __ffs(absent) - 1;
+                absent &= absent - 1;
+                colo[k] = (d + B) * WE;
+                orec[k] = __popc(RQ & ((1u << d) - 1u)) * L.cnt_next + L.rank16[SQ | (1u << d)];
+            } else {
+                colo[k] = h * WE;      // dummy target
+                orec[k] = -1;
+            }
         }
         colo[N] = h * WE;
     }
@@ -248,6 +255,7 @@ __device__ __forceinline__ void team_item(const TeamLevel& L, unsigned SQ, int x
     // ---- outputs: next-level records, and Z[(SQ, R_T)] = -close (one -1 per closed fermion loop) ----
 #pragma unroll
     for (int k = 0; k < N; ++k) {
+        if (orec[k] < 0) continue;
         const RecPtr<C> o(sm + L.off_nxt, orec[k]);
 #pragma unroll
         for (int p = 0; p < 4; ++p)
@@ -262,9 +270,13 @@ __device__ __forceinline__ void team_item(const TeamLevel& L, unsigned SQ, int x
 }
 
 template <int C>
-__device__ __forceinline__ void team_dispatch_item(const TeamLevel& L, unsigned SQ, int x, double* sm, const double* Wl)
+__device__ __forceinline__ void team_dispatch_item(const TeamLevel& L, unsigned SQ, int x, double* sm, const double* Wl,
+                                                   bool active)
 {
-    const int N = (31 - __clz((int)SQ)) - L.j;
+    // warp-uniform target count: the widest item of the warp (all 32 lanes call this)
+    const int Nown = active ? (31 - __clz((int)SQ)) - L.j : 0;
+    const int N = __reduce_max_sync(0xffffffffu, Nown);
+    if (!active) return;
     switch (N) {
         case 0: team_item<C, 0>(L, SQ, x, sm, Wl); break;
         case 1: team_item<C, 1>(L, SQ, x, sm, Wl); break;
@@ -616,8 +628,11 @@ __global__ void __launch_bounds__(MAXT, MINB) eval_team_kernel(EvalArgs a, TeamD
             L.lvlZ_j = lvlZ[j]; L.lvlZ_j1 = lvlZ[j + 1];
             L.off_cur = cur; L.off_nxt = nxt;
             const uint16_t* masks = mask16 + lvlT[j + 1];
-            for (int x = slot; x < L.cnt; x += d.pslots)
-                if (g < ninst) team_dispatch_item<C>(L, masks[x], x, sm, Wl);
+            for (int x0 = 0; x0 < L.cnt; x0 += d.pslots) {
+                const int x = x0 + slot;
+                const bool active = (x < L.cnt) && (g < ninst);
+                team_dispatch_item<C>(L, active ? masks[x] : 1u, x, sm, Wl, active);
+            }
             __syncthreads();
             const int tmp = cur; cur = nxt; nxt = tmp;
         }
