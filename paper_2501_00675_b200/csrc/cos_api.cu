@@ -277,7 +277,7 @@ int cos_eval_connected_xt(cos_ctx* c, int n, long long batch, const int* d_xy, c
     c->last_launches = 0;
     if (batch == 0) return COS_OK;
     const bool two = c->table[1] && c->table[1] != c->table[0];
-    if (uses_team(n) && team_choice(n, two ? 2 : 1).d.smem_bytes <= (size_t)c->smem_optin) {
+    if (has_fused_kernel(n, two ? 2 : 1, c->smem_optin)) {
         // a1 fused into the evaluation kernel: G is assembled straight into shared memory
         EvalArgs a{};
         a.n = n; a.batch = batch; a.u = d_u; a.U = U; a.out = d_out; a.connected = 1; a.off = c->off;
@@ -386,11 +386,11 @@ long long cos_flop_count(int n, int n_species, int connected)
 #ifdef COS_PHASE_TIMING
 // Development aid (not part of include/cos.h; compiled only with -DCOS_PHASE_TIMING): cycles thread 0 of every
 // CTA spent in each phase of the evaluation kernels, summed over CTAs.
-extern "C" int cos_debug_phase_cycles(unsigned long long* h_out8, int reset)
+extern "C" int cos_debug_phase_cycles(unsigned long long* h_out32, int reset)
 {
-    if (h_out8 && cudaMemcpyFromSymbol(h_out8, cosb::g_phase_cycles, 8 * sizeof(unsigned long long)) != cudaSuccess) return COS_ECUDA;
+    if (h_out32 && cudaMemcpyFromSymbol(h_out32, cosb::g_phase_cycles, 32 * sizeof(unsigned long long)) != cudaSuccess) return COS_ECUDA;
     if (reset) {
-        unsigned long long z[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+        unsigned long long z[32] = {0};
         if (cudaMemcpyToSymbol(cosb::g_phase_cycles, z, sizeof(z)) != cudaSuccess) return COS_ECUDA;
     }
     return COS_OK;

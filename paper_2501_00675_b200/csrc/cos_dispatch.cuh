@@ -4,6 +4,7 @@
 #include "cos_kernels_generic.cuh"
 #include "cos_kernels_tiled.cuh"
 #include "cos_kernels_team.cuh"
+#include "cos_kernels_pair.cuh"
 
 namespace cosb {
 
@@ -79,6 +80,26 @@ inline TeamChoice team_choice(int n, int nsp)
     return {eval_team_kernel<32, 192, 2>, team_dims<32>(n, nsp)};
 }
 
+// ---- pair kernel (orders 11..12): the team mapping with every item split over a lane pair ----
+constexpr int kPairMinN = 11, kPairMaxN = 12;
+using PairKernel = void (*)(EvalArgs, PairDims);
+struct PairChoice { PairKernel fn; PairDims d; };
+inline bool uses_pair(int n) { return n >= kPairMinN && n <= kPairMaxN; }
+// True when order n has a kernel that assembles G on the fly (cos_eval_connected_xt without a G round trip).
+inline bool has_fused_kernel(int n, int nsp, int smem_optin);
+inline PairChoice pair_choice(int n, int nsp)
+{
+    if (n == 12) return {eval_pair_kernel<2, 512, 1, 9>, pair_dims<2>(n, nsp)};
+    return {eval_pair_kernel<4, 576, 1, 8>, pair_dims<4>(n, nsp)};
+}
+
+inline bool has_fused_kernel(int n, int nsp, int smem_optin)
+{
+    if (uses_team(n)) return team_choice(n, nsp).d.smem_bytes <= (size_t)smem_optin;
+    if (uses_pair(n)) return pair_choice(n, nsp).d.smem_bytes <= (size_t)smem_optin;
+    return false;
+}
+
 using TiledKernel = void (*)(EvalArgs, TiledDims);
 inline TiledKernel tiled_kernel() { return eval_tiled_kernel<kTiledB, kTiledThreads, kTiledNA, kTiledJB, false>; }
 inline TiledKernel big_kernel() { return eval_tiled_kernel<kTiledB, kBigThreads, kBigNA, kBigJB, true>; }
@@ -90,6 +111,10 @@ inline cudaError_t configure_kernels(int smem_optin)
     if (e != cudaSuccess) return e;
     for (int n = kTeamMinN; n <= kTeamMaxN; ++n) {
         e = cudaFuncSetAttribute(team_choice(n, 1).fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
+        if (e != cudaSuccess) return e;
+    }
+    for (int n = kPairMinN; n <= kPairMaxN; ++n) {
+        e = cudaFuncSetAttribute(pair_choice(n, 1).fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
         if (e != cudaSuccess) return e;
     }
     e = cudaFuncSetAttribute(big_kernel(), cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
@@ -117,7 +142,22 @@ inline cudaError_t dispatch_eval(const EvalArgs& a, cudaStream_t stream, int num
             return cudaGetLastError();
         }
     }
-    if (a.fused) return cudaErrorInvalidValue;   // only the team kernel assembles G on the fly
+    if (uses_pair(a.n)) {
+        const PairChoice tc = pair_choice(a.n, nsp);
+        if (tc.d.smem_bytes <= (size_t)smem_optin) {
+            int per_sm = 1;
+            cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, tc.fn, tc.d.threads, tc.d.smem_bytes);
+            if (e != cudaSuccess) return e;
+            if (per_sm < 1) per_sm = 1;
+            const long long teams = (a.batch * nsp + tc.d.C - 1) / tc.d.C;
+            long long grid = (long long)num_sms * per_sm;
+            if (grid > teams) grid = teams;
+            tc.fn<<<(unsigned)grid, tc.d.threads, tc.d.smem_bytes, stream>>>(a, tc.d);
+            *name = "eval_pair_kernel";
+            return cudaGetLastError();
+        }
+    }
+    if (a.fused) return cudaErrorInvalidValue;   // only the team and pair kernels assemble G on the fly
     if (uses_big(a.n)) {
         const TiledDims d = big_dims(a.n, nsp);
         const size_t smem = (size_t)d.tab_bytes;

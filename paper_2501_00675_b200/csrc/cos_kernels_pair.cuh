@@ -1,0 +1,490 @@
+// cos_kernels_pair.cuh -- "pair" CoS evaluation kernel (orders 5..12): the team mapping of cos_kernels_team.cuh
+// with every work item split over a PAIR of adjacent lanes.
+//
+// What is computed is unchanged: vertices are split into T = {0,1,2} and Q = {3..n-1}; a work
+// item is one Q-pattern S_Q of one propagation instance (configuration x species); all stages advance together,
+// level j holds the patterns with |S_Q| = j + 1; a node record (S_Q, c) is the 8 values R_T subset of T.
+//
+// What changes is who holds what.  The measured limit of the team kernel was latency, not arithmetic: one
+// thread carried the whole 8 x (N+1) register tile of a pattern, so a level exposed at most 35 x C threads of
+// work, each with a long dependent instruction stream, and the block barrier of every level waited for it.
+// Here the two lanes (2i, 2i+1) of a pair share one item and split its ROWS: lane u holds the R_T subsets
+// t = 4u + r, r = 0..3 (vertex 2 absent / present):
+//   * each lane loads only its half of a source record (2 x LDS.128 instead of 4) -- no duplicated traffic;
+//   * both lanes read the same W entries; the shared-memory pipeline merges identical addresses of adjacent
+//     lanes (measured: LDS.64 with pairwise equal addresses costs 1 cycle per warp instead of 2), so the W
+//     gather costs half as many wavefronts as with one lane per item;
+//   * transitions inside T' = {0,1} stay inside a lane; the 4 nodes (t, 2) that cross from lane 0 to lane 1
+//     are exchanged with one round of shuffles per item;
+//   * per-thread work and registers halve, the number of resident threads doubles.
+// Shared-memory layout (doubles), lane fastest so that one quarter warp touches one contiguous 128-byte row:
+//   record rec, chunk p in {0,1}, instance g, lane half u:   rec * 8C + p * 4C + (2g + u) * 2 + e
+//   holds the value of R_T = t = 4u + 2p + e.  For C = 2 (two items per quarter warp) p is XOR-ed with the
+//   parity of rec, which differs between the records two neighbouring patterns read at the same time.
+//   W entry (c, c') of instance g, replica r:                (c * n + c') * 16 + r * C + g     (16 / C replicas)
+#pragma once
+#include "cos_common.cuh"
+#include "cos_kernels_generic.cuh"
+#include "cos_kernels_tiled.cuh"   // kBinom, cpopc
+#include "cos_kernels_team.cuh"    // RedLayout, team_reduce (connected reduction on interleaved blocks)
+
+namespace cosb {
+
+constexpr int kPairB = 3;            // |T|
+constexpr int kPairMaxCols = 9;      // Q-targets + close held in registers (order 12: at most 8 + 1)
+
+template <int C> struct PairLayout {
+    static_assert(C == 2 || C == 4 || C == 8 || C == 16, "instances per team");
+    static constexpr int REP = 16 / C;           // W replicas: the 16 pairs of a warp read 16 distinct banks
+    static constexpr int WE = 16;                // doubles per W entry (REP * C)
+    static constexpr int CH = 4 * C;             // doubles per record chunk
+    static constexpr int REC = 8 * C;            // doubles per node record
+    static constexpr int SWZ = (C == 2) ? 1 : 0; // chunk swizzle by record parity
+    static constexpr int PW = 16 / C;            // patterns per warp
+};
+
+// Double offset of chunk p of record rec (without the lane part).
+template <int C>
+__device__ __forceinline__ int pair_chunk(int rec, int p)
+{
+    using L = PairLayout<C>;
+    return rec * L::REC + (L::SWZ ? ((p ^ rec) & 1) : p) * L::CH;
+}
+
+struct PairDims {
+    int n, nsp, C;
+    int qmax;          // n - 3
+    int pslots;        // pattern slots per pass = threads / (2C)
+    int threads;
+    int maxrec;        // records per frontier buffer
+    int zrec;          // Z records (2^qmax)
+    int ncfg;          // configuration slots of a team = C / nsp
+    int red_rows;      // 2^(n-1-kRedLB) block rows of the reduction arrays
+    int off_w, off_u, off_z, off_b0, off_b1;   // double offsets behind the tables
+    int off_cb, off_db;                        // reduction arrays (alias the frontier buffers)
+    int tab_bytes;
+    size_t smem_bytes;
+};
+
+template <int C>
+inline PairDims pair_dims(int n, int nsp)
+{
+    using L = PairLayout<C>;
+    PairDims d{};
+    d.n = n; d.nsp = nsp; d.C = C;
+    d.qmax = n - kPairB;
+    int slots = team_max_patterns(n);
+    slots = (slots + L::PW - 1) / L::PW * L::PW;
+    if (slots * 2 * C < 64) slots = 64 / (2 * C);
+    d.pslots = slots;
+    d.threads = slots * 2 * C;
+    int rec_even = 1, rec_odd = 1;                        // ping-pong buffers sized for the levels they hold
+    for (int j = 0; j <= d.qmax; ++j) {
+        const int v = j * kBinomHost.c[d.qmax][j + 1];
+        if (j & 1) { if (v > rec_odd) rec_odd = v; } else { if (v > rec_even) rec_even = v; }
+    }
+    d.maxrec = rec_even > rec_odd ? rec_even : rec_odd;
+    d.zrec = 1 << d.qmax;
+    d.ncfg = C / nsp;
+    d.red_rows = 1 << (n - 1 - kRedLB);
+    d.off_w = 0;
+    d.off_u = d.off_w + n * n * L::WE;
+    d.off_z = d.off_u + 16 * d.ncfg;                      // un[v][cfg] = -u_v
+    d.off_b0 = d.off_z + d.zrec * L::REC;
+    d.off_b1 = d.off_b0 + rec_even * L::REC;              // level j reads buffer (j & 1), writes buffer (~j & 1)
+    int work = (rec_even + rec_odd) * L::REC;
+    const int need = 2 * d.red_rows * 16 * d.ncfg;
+    if (work < need) work = need;
+    d.off_cb = d.off_b0;
+    d.off_db = d.off_b0 + d.red_rows * 16 * d.ncfg;
+    d.tab_bytes = ((2 * 2 * (1 << (n - 1)) + 4 * 64 + 2 * d.zrec) + 15) & ~15;   // mask16, rank16, lvlT, lvlZ, recSQ
+    d.smem_bytes = (size_t)d.tab_bytes + sizeof(double) * (size_t)(d.off_b0 + work);
+    return d;
+}
+
+// Uniform description of one level step.
+struct PairLevel {
+    int n, j;
+    int cnt, cnt_next;          // patterns at levels j and j + 1
+    int lvlZ_j, lvlZ_j1;        // Z record offsets of |S_Q| = j and j + 1
+    int off_z, off_cur, off_nxt;
+    const uint16_t* rank16;
+};
+
+// The 4 values (rows r = 0..3 of this lane half) of record rec.  sm already carries the lane part.
+template <int C>
+__device__ __forceinline__ void pair_load_rec(const double* sm, int rec, double (&a)[4])
+{
+    const double2 v0 = *reinterpret_cast<const double2*>(sm + pair_chunk<C>(rec, 0));
+    const double2 v1 = *reinterpret_cast<const double2*>(sm + pair_chunk<C>(rec, 1));
+    a[0] = v0.x; a[1] = v0.y; a[2] = v1.x; a[3] = v1.y;
+}
+
+template <int C>
+__device__ __forceinline__ void pair_store_rec(double* sm, int rec, double a0, double a1, double a2, double a3)
+{
+    *reinterpret_cast<double2*>(sm + pair_chunk<C>(rec, 0)) = make_double2(a0, a1);
+    *reinterpret_cast<double2*>(sm + pair_chunk<C>(rec, 1)) = make_double2(a2, a3);
+}
+
+// One item: Q-pattern SQ (|SQ| = j + 1, top element q, stage vertex h = q + 3) of one instance, rows 4u..4u+3.
+//   sm : shared doubles, already offset by the lane part (2g + u) * 2
+//   Wl : W of this instance and replica, entry (c, c') at Wl[(c * n + c') * 16]
+// NC = N + 1 columns are accumulated in registers: the N = q - j Q-targets and the close (column h), together
+// with the 8 T-target accumulators.  NC is the widest item of the WARP (warp-uniform, the dispatch never
+// diverges); an item with fewer targets pads with dummy columns that read a valid W column and are never stored.
+template <int C, int NC>
+__device__ __forceinline__ void pair_item(const PairLevel& L, unsigned SQ, int x, int u, double* sm, const double* Wl,
+                                          unsigned lanes)
+{
+    constexpr int WE = PairLayout<C>::WE, B = kPairB, N = NC - 1;
+    const int n = L.n;
+    const int q = 31 - __clz((int)SQ);
+    const unsigned RQ = SQ ^ (1u << q);
+    const int h = q + B;
+    int colo[NC];                     // W column offset of column k; the last one is the close column h
+    int orec[N > 0 ? N : 1];          // record number of target k in the next buffer
+    {
+        unsigned absent = ~RQ & ((1u << q) - 1u);
+#pragma unroll
+        for (int k = 0; k < N; ++k) {
+            if (absent) {
+                const int d = __ffs(absent) - 1;
+                absent &= absent - 1;
+                colo[k] = (d + B) * WE;
+                orec[k] = __popc(RQ & ((1u << d) - 1u)) * L.cnt_next + L.rank16[SQ | (1u << d)];
+            } else {
+                colo[k] = h * WE;      // dummy column
+                orec[k] = -1;
+            }
+        }
+        colo[N] = h * WE;
+    }
+    const int rowstride = n * WE;
+    double acc[4][NC];
+    double T00, T01, T11, T20, T02, T12, T22, T32;     // T_{r,tp}: node (R_T = t + {tp}, tp), t = 4u + r
+    // ---- the start node (S, h) = Z[S \ {h}] ("top node", one per stage) ----
+    {
+        double a[4];
+        pair_load_rec<C>(sm + L.off_z, L.lvlZ_j + L.rank16[RQ], a);
+        const double* row = Wl + h * rowstride;
+#pragma unroll
+        for (int k = 0; k < NC; ++k) {
+            const double w = row[colo[k]];
+#pragma unroll
+            for (int r = 0; r < 4; ++r) acc[r][k] = a[r] * w;
+        }
+        const double w0 = row[0], w1 = row[WE], w2 = row[2 * WE];
+        T00 = a[0] * w0; T20 = a[2] * w0;
+        T01 = a[0] * w1; T11 = a[1] * w1;
+        T02 = a[0] * w2; T12 = a[1] * w2; T22 = a[2] * w2; T32 = a[3] * w2;
+    }
+    // ---- sources in Q, streamed from the level buffer ----
+    {
+        unsigned m = RQ;
+        int rec = x;
+        for (int i = 0; i < L.j; ++i) {
+            const int v = __ffs(m) - 1 + B;
+            m &= m - 1;
+            double a[4];
+            pair_load_rec<C>(sm + L.off_cur, rec, a);
+            rec += L.cnt;
+            const double* row = Wl + v * rowstride;
+#pragma unroll
+            for (int k = 0; k < NC; ++k) {
+                const double w = row[colo[k]];
+#pragma unroll
+                for (int r = 0; r < 4; ++r) acc[r][k] = fma(a[r], w, acc[r][k]);
+            }
+            const double w0 = row[0], w1 = row[WE], w2 = row[2 * WE];
+            T00 = fma(a[0], w0, T00); T20 = fma(a[2], w0, T20);
+            T01 = fma(a[0], w1, T01); T11 = fma(a[1], w1, T11);
+            T02 = fma(a[0], w2, T02); T12 = fma(a[1], w2, T12); T22 = fma(a[2], w2, T22); T32 = fma(a[3], w2, T32);
+        }
+    }
+    // ---- transitions inside T.  Lane 0 (vertex 2 absent) first completes its nodes (t, 2); they are the nodes
+    //      (4 + r, 2) of lane 1, which receives them by shuffle and then completes its own T' = {0,1} nodes. ----
+    const double W01 = Wl[(0 * n + 1) * WE], W02 = Wl[(0 * n + 2) * WE];
+    const double W10 = Wl[(1 * n + 0) * WE], W12 = Wl[(1 * n + 2) * WE];
+    const double W20 = Wl[(2 * n + 0) * WE], W21 = Wl[(2 * n + 1) * WE];
+    if (u == 0) {
+        T11 = fma(T00, W01, T11); T20 = fma(T01, W10, T20);
+        T12 = fma(T00, W02, T12); T22 = fma(T01, W12, T22);
+        T32 = fma(T20, W02, fma(T11, W12, T32));
+    }
+    double X0 = __shfl_xor_sync(lanes, T02, 1), X1 = __shfl_xor_sync(lanes, T12, 1);
+    double X2 = __shfl_xor_sync(lanes, T22, 1), X3 = __shfl_xor_sync(lanes, T32, 1);
+    if (u == 0) {
+        X0 = 0.0; X1 = 0.0; X2 = 0.0; X3 = 0.0;
+    } else {
+        T00 = fma(X0, W20, T00); T01 = fma(X0, W21, T01);
+        T11 = fma(X1, W21, T11); T20 = fma(X2, W20, T20);
+        T11 = fma(T00, W01, T11); T20 = fma(T01, W10, T20);
+    }
+    // ---- sources in T -> Q-targets and the close ----
+#pragma unroll
+    for (int k = 0; k < NC; ++k) {
+        const double w0 = Wl[colo[k]], w1 = Wl[rowstride + colo[k]], w2 = Wl[2 * rowstride + colo[k]];
+        acc[0][k] = fma(X0, w2, acc[0][k]);
+        acc[1][k] = fma(X1, w2, fma(T00, w0, acc[1][k]));
+        acc[2][k] = fma(X2, w2, fma(T01, w1, acc[2][k]));
+        acc[3][k] = fma(X3, w2, fma(T20, w0, fma(T11, w1, acc[3][k])));
+    }
+    // ---- outputs: next-level records, and Z[(SQ, R_T)] = -close (one -1 per closed fermion loop) ----
+#pragma unroll
+    for (int k = 0; k < N; ++k) {
+        if (orec[k] < 0) continue;
+        pair_store_rec<C>(sm + L.off_nxt, orec[k], acc[0][k], acc[1][k], acc[2][k], acc[3][k]);
+    }
+    pair_store_rec<C>(sm + L.off_z, L.lvlZ_j1 + x, -acc[0][N], -acc[1][N], -acc[2][N], -acc[3][N]);
+}
+
+template <int C, int MAXNC>
+__device__ __forceinline__ void pair_dispatch_item(const PairLevel& L, unsigned SQ, int x, int u, double* sm,
+                                                   const double* Wl, bool active)
+{
+    // warp-uniform column count: the widest item of the warp (all 32 lanes call this)
+    const int Nown = active ? (31 - __clz((int)SQ)) - L.j : 0;
+    const int N = __reduce_max_sync(0xffffffffu, Nown);
+    // both lanes of a pair are active together, so the shuffles inside an item see their partner
+    const unsigned lanes = __ballot_sync(0xffffffffu, active);
+    if (!active) return;
+#define COS_PAIR_CASE(K) case K - 1: if (K <= MAXNC) { pair_item<C, (K <= MAXNC ? K : 1)>(L, SQ, x, u, sm, Wl, lanes); break; }
+    switch (N) {
+        COS_PAIR_CASE(1) COS_PAIR_CASE(2) COS_PAIR_CASE(3) COS_PAIR_CASE(4) COS_PAIR_CASE(5)
+        COS_PAIR_CASE(6) COS_PAIR_CASE(7) COS_PAIR_CASE(8)
+        default: pair_item<C, MAXNC>(L, SQ, x, u, sm, Wl, lanes); break;
+    }
+#undef COS_PAIR_CASE
+}
+
+// Z[(SQ = {}, R_T)] for the 8 subsets of T (stages h < 3), one thread per instance, in the propagation's own
+// order (start / extend / close).  Wl: W of this instance (any replica); zr: Z record 0 + 4g doubles.
+template <int C>
+__device__ __forceinline__ void pair_small_stages(const double* Wl, int n, double* zr)
+{
+    constexpr int WE = PairLayout<C>::WE;
+    auto W = [&](int a, int b) { return Wl[(a * n + b) * WE]; };
+    const double w00 = W(0, 0), w01 = W(0, 1), w02 = W(0, 2);
+    const double w10 = W(1, 0), w11 = W(1, 1), w12 = W(1, 2);
+    const double w20 = W(2, 0), w21 = W(2, 1), w22 = W(2, 2);
+    double z[8];
+    z[0] = 1.0;                                           // top node
+    z[1] = -w00;                                          // stage 0
+    z[2] = -w11;                                          // stage 1, R = {}
+    z[3] = -fma(w10, w01, z[1] * w11);                    // stage 1, R = {0}: nodes (R,0) = W[1][0], (R,1) = Z[{0}]
+    z[4] = -w22;                                          // stage 2, R = {}
+    z[5] = -fma(w20, w02, z[1] * w22);                    // R = {0}
+    z[6] = -fma(w21, w12, z[2] * w22);                    // R = {1}
+    const double p01_1 = fma(w20, w01, z[1] * w21);       // node ({0,1}, 1) from R = {0}
+    const double p01_0 = fma(w21, w10, z[2] * w20);       // node ({0,1}, 0) from R = {1}
+    z[7] = -fma(p01_0, w02, fma(p01_1, w12, z[3] * w22)); // R = {0,1}
+#pragma unroll
+    for (int uu = 0; uu < 2; ++uu)
+#pragma unroll
+        for (int p = 0; p < 2; ++p)                       // record 0: chunk p, value t = 4u + 2p + e
+            *reinterpret_cast<double2*>(zr + pair_chunk<C>(0, p) + uu * 2) = make_double2(z[4 * uu + 2 * p], z[4 * uu + 2 * p + 1]);
+}
+
+// a3: D[S] = w(S) Zup[S] Zdn[S] for the NC configurations of the team, written straight into the reduction
+// arrays: S odd -> CB (D0[S >> 1]), S even -> DB (D1[S >> 1]).  One thread per (Z record, configuration): the 8
+// values R_T of record S_Q are the lo-values (S_Q & 3) * 4 + {0..3} of row hi = S_Q >> 2 in both arrays.
+// un[v * NC + cg] = -u_v of configuration cg (aliased species only; otherwise -u is folded into W).
+template <int C, int NC>
+__device__ __forceinline__ void pair_combine(double* smd, const PairDims& d, int ncfg, const uint16_t* recSQ,
+                                             int tid, int nthreads)
+{
+    using R = RedLayout<NC>;
+    constexpr int NSP = C / NC;
+    double* CB = smd + d.off_cb;
+    double* DB = smd + d.off_db;
+    const double* un = smd + d.off_u;
+    const int cg = tid % NC;
+    if (cg >= ncfg) return;
+    double wT[8];
+#pragma unroll
+    for (int t = 0; t < 8; ++t) wT[t] = 1.0;
+    if (NSP == 1) {
+        const double u0 = un[0 * NC + cg], u1 = un[1 * NC + cg], u2 = un[2 * NC + cg];
+#pragma unroll
+        for (int t = 0; t < 8; ++t) wT[t] = ((t & 1) ? u0 : 1.0) * ((t & 2) ? u1 : 1.0) * ((t & 4) ? u2 : 1.0);
+    }
+    for (int rec = tid / NC; rec < d.zrec; rec += nthreads / NC) {
+        const unsigned SQ = recSQ[rec];
+        double wq = 1.0;
+        if (NSP == 1) {
+            unsigned m = SQ;
+            while (m) { const int v = __ffs(m) - 1; m &= m - 1; wq *= un[(v + kPairB) * NC + cg]; }
+        }
+        const double* zup = smd + d.off_z + (cg * NSP) * 4;
+        const double* zdn = smd + d.off_z + (cg * NSP + NSP - 1) * 4;
+        double val[8];
+#pragma unroll
+        for (int pi = 0; pi < 4; ++pi) {                  // values t = 2 pi, 2 pi + 1: lane half pi >> 1, chunk pi & 1
+            const int o = pair_chunk<C>(rec, pi & 1) + (pi >> 1) * 2;
+            const double2 zu = *reinterpret_cast<const double2*>(zup + o);
+            const double2 zd = *reinterpret_cast<const double2*>(zdn + o);
+            val[2 * pi] = (wq * wT[2 * pi]) * (zu.x * zd.x);
+            val[2 * pi + 1] = (wq * wT[2 * pi + 1]) * (zu.y * zd.y);
+        }
+        const unsigned hi = SQ >> 2;
+        const int pa = (int)(SQ & 3u) * 2, sw = red_swz<NC>(hi);
+        double* crow = CB + (int)hi * R::ROW + cg * 2;
+        double* drow = DB + (int)hi * R::ROW + cg * 2;
+        *reinterpret_cast<double2*>(crow + ((pa) ^ sw) * R::PSTR) = make_double2(val[1], val[3]);
+        *reinterpret_cast<double2*>(crow + ((pa + 1) ^ sw) * R::PSTR) = make_double2(val[5], val[7]);
+        *reinterpret_cast<double2*>(drow + ((pa) ^ sw) * R::PSTR) = make_double2(val[0], val[2]);
+        *reinterpret_cast<double2*>(drow + ((pa + 1) ^ sw) * R::PSTR) = make_double2(val[4], val[6]);
+    }
+}
+
+// One team's W matrices into shared memory (a1 fused, or a load of materialised G), instance fastest; -u_a is
+// folded into the rows of species 0 when the species are distinct.  Entry e of instance gi, replica r at
+// e * 16 + r * C + gi.
+template <int C>
+__device__ __forceinline__ void pair_load_w(const EvalArgs& a, const PairDims& d, double* smd, long long inst0, int ninst,
+                                            int tid, int nthreads)
+{
+    using Lay = PairLayout<C>;
+    const int n = d.n, nsp = d.nsp;
+    for (int t = tid; t < C * n * n; t += nthreads) {
+        const int gi = t % C, e = t / C;
+        double val = 0.0;
+        if (gi < ninst) {
+            const long long b = (inst0 + gi) / nsp;
+            const int s = (int)((inst0 + gi) % nsp);
+            if (a.fused) {
+                double gu, gd;
+                g0_entry(a.bg, b, e / n, e % n, gu, gd);
+                val = s ? gd : gu;
+            } else {
+                val = (s == 0 ? a.Gup : a.Gdn)[b * n * n + e];
+            }
+            if (nsp == 2 && s == 0) val *= -(a.u ? a.u[b * n + e / n] : a.U);
+        }
+        double* w = smd + d.off_w + e * Lay::WE + gi;
+#pragma unroll
+        for (int r = 0; r < Lay::REP; ++r) w[r * C] = val;
+    }
+    if (nsp == 1) {     // un[v][cfg] = -u_v (aliased species only: w(S) is applied in the combine step)
+        const int NCt = C, ncfg = ninst;
+        for (int t = tid; t < NCt * n; t += nthreads) {
+            const int cg = t % NCt, v = t / NCt;
+            smd[d.off_u + v * NCt + cg] = (cg < ncfg) ? -(a.u ? a.u[(inst0 + cg) * n + v] : a.U) : 0.0;
+        }
+    }
+}
+
+template <int C, int MAXT, int MINB, int MAXNC>
+__global__ void __launch_bounds__(MAXT, MINB) eval_pair_kernel(EvalArgs a, PairDims d)
+{
+    using Lay = PairLayout<C>;
+    constexpr int WE = Lay::WE, REP = Lay::REP;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+#ifdef COS_PHASE_TIMING
+    long long phase_t0__ = clock64();
+#endif
+    uint16_t* mask16 = reinterpret_cast<uint16_t*>(smem_raw);
+    uint16_t* rank16 = mask16 + (1 << (d.n - 1));
+    int* lvlT = reinterpret_cast<int*>(rank16 + (1 << (d.n - 1)));   // list offsets, ground set n-1 bits
+    int* lvlZ = lvlT + 32;                                           // Z record offsets, ground set qmax bits
+    uint16_t* recSQ = reinterpret_cast<uint16_t*>(lvlZ + 32);        // Z record -> S_Q
+    double* smd = reinterpret_cast<double*>(smem_raw + d.tab_bytes);
+    const int tid = threadIdx.x, nthreads = blockDim.x;
+    const int n = d.n, qmax = d.qmax, nsp = d.nsp;
+    const unsigned NS = 1u << n;
+    const int u = tid & 1;                       // lane half: vertex 2 absent / present in this lane's rows
+    const int g = (tid >> 1) % C;                // instance of this thread
+    const int slot = tid / (2 * C);              // pattern slot
+    const int rep = slot % REP;                  // W replica read by this thread
+    double* sm = smd + (2 * g + u) * 2;
+    const double* Wl = smd + d.off_w + rep * C + g;
+
+    // ---- tables: subsets of {0..n-2} by popcount in colex order (rank independent of the ground set) ----
+    if (tid == 0) {
+        int run = 0;
+        for (int j = 0; j <= n; ++j) { lvlT[j] = run; run += kBinom.c[n - 1][j]; }
+        run = 0;
+        for (int j = 0; j <= qmax + 1; ++j) { lvlZ[j] = run; run += kBinom.c[qmax][j]; }
+    }
+    __syncthreads();
+    for (unsigned mk = tid; mk < (1u << (n - 1)); mk += nthreads) {
+        int rk = 0, i = 0;
+        unsigned m = mk;
+        while (m) { const int s = __ffs(m) - 1; m &= m - 1; ++i; rk += kBinom.c[s][i]; }
+        rank16[mk] = (uint16_t)rk;
+        mask16[lvlT[i] + rk] = (uint16_t)mk;
+        if (mk < (1u << qmax)) recSQ[lvlZ[i] + rk] = (uint16_t)mk;
+    }
+    __syncthreads();
+
+    const long long total_inst = a.batch * nsp;
+    const long long nteams = (total_inst + C - 1) / C;
+    for (long long team = blockIdx.x; team < nteams; team += gridDim.x) {
+        const long long inst0 = team * C;
+        const int ninst = (int)min((long long)C, total_inst - inst0);
+        const int ncfg = ninst / nsp;
+        const long long cfgbase = inst0 / nsp;
+        __syncthreads();
+        pair_load_w<C>(a, d, smd, inst0, ninst, tid, nthreads);
+        __syncthreads();
+        COS_PHASE_MARK(0);
+        if (tid < ninst) pair_small_stages<C>(smd + d.off_w + tid, n, smd + d.off_z + tid * 4);
+        __syncthreads();
+        COS_PHASE_MARK(1);
+
+        // ---- a2: all stages together, level j = |S_Q| - 1; level j reads buffer (j & 1) and writes the other ----
+        PairLevel L;
+        L.n = n; L.rank16 = rank16; L.off_z = d.off_z;
+        for (int j = 0; j < qmax; ++j) {
+            L.j = j;
+            L.cnt = kBinom.c[qmax][j + 1];
+            L.cnt_next = kBinom.c[qmax][j + 2];
+            L.lvlZ_j = lvlZ[j]; L.lvlZ_j1 = lvlZ[j + 1];
+            L.off_cur = (j & 1) ? d.off_b1 : d.off_b0;
+            L.off_nxt = (j & 1) ? d.off_b0 : d.off_b1;
+            const uint16_t* masks = mask16 + lvlT[j + 1];
+            for (int x0 = 0; x0 < L.cnt; x0 += d.pslots) {
+                const int x = x0 + slot;
+                const bool active = (x < L.cnt) && (g < ninst);
+                pair_dispatch_item<C, MAXNC>(L, active ? masks[x] : 1u, x, u, sm, Wl, active);
+            }
+            __syncthreads();
+            COS_PHASE_MARK(2 + j);
+        }
+
+        // ---- a3 + a5 ("all"): D[full] = w * Zup[full] * Zdn[full]; S_Q = Q, R_T = T: lane half 1, chunk 1, e = 1 ----
+        if (!a.connected) {
+            if (tid < ncfg) {
+                const double* zp = smd + d.off_z + pair_chunk<C>(lvlZ[qmax], 1) + 2 + 1;
+                const double zu = zp[(tid * nsp) * 4];
+                const double zd = zp[(tid * nsp + nsp - 1) * 4];
+                double w = 1.0;
+                if (nsp == 1) for (int v = 0; v < n; ++v) w *= smd[d.off_u + v * C + tid];
+                a.out[cfgbase + tid] = w * zu * zd;
+            }
+            continue;
+        }
+
+        // ---- a3: combine, a4: connected reduction, a5: C'[full] ----
+        double* CB = smd + d.off_cb;
+        const double* DB = smd + d.off_db;
+        if (nsp == 1) {
+            pair_combine<C, C>(smd, d, ncfg, recSQ, tid, nthreads);
+            __syncthreads();
+            COS_PHASE_MARK(12);
+            team_reduce<C>(CB, DB, ncfg, n, mask16, lvlT, tid, nthreads);
+            COS_PHASE_MARK(13);
+            if (tid < ncfg) a.out[cfgbase + tid] = CB[red_elem<C>((NS >> (1 + kRedLB)) - 1, 15u, tid)];
+        } else {
+            pair_combine<C, C / 2>(smd, d, ncfg, recSQ, tid, nthreads);
+            __syncthreads();
+            COS_PHASE_MARK(12);
+            team_reduce<C / 2>(CB, DB, ncfg, n, mask16, lvlT, tid, nthreads);
+            COS_PHASE_MARK(13);
+            if (tid < ncfg) a.out[cfgbase + tid] = CB[red_elem<C / 2>((NS >> (1 + kRedLB)) - 1, 15u, tid)];
+        }
+    }
+}
+
+}  // namespace cosb

@@ -543,6 +543,9 @@ __global__ void __launch_bounds__(MAXT, MINB) eval_team_kernel(EvalArgs a, TeamD
     using Lay = TeamLayout<C>;
     constexpr int WE = Lay::WE, REC = Lay::REC, PART = Lay::PART, REP = Lay::REP;
     extern __shared__ __align__(16) unsigned char smem_raw[];
+#ifdef COS_PHASE_TIMING
+    long long phase_t0__ = clock64();
+#endif
     uint16_t* mask16 = reinterpret_cast<uint16_t*>(smem_raw);
     uint16_t* rank16 = mask16 + (1 << (d.n - 1));
     int* lvlT = reinterpret_cast<int*>(rank16 + (1 << (d.n - 1)));   // list offsets, ground set n-1 bits
@@ -614,8 +617,10 @@ __global__ void __launch_bounds__(MAXT, MINB) eval_team_kernel(EvalArgs a, TeamD
             }
         }
         __syncthreads();
+        COS_PHASE_MARK(0);
         if (tid < ninst) team_small_stages<C>(smd + d.off_w + tid, n, smd + d.off_z + tid * 2);
         __syncthreads();
+        COS_PHASE_MARK(1);
 
         // ---- a2: all stages together, level j = |S_Q| - 1 ----
         TeamLevel L;
@@ -634,6 +639,7 @@ __global__ void __launch_bounds__(MAXT, MINB) eval_team_kernel(EvalArgs a, TeamD
                 team_dispatch_item<C>(L, active ? masks[x] : 1u, x, sm, Wl, active);
             }
             __syncthreads();
+            COS_PHASE_MARK(2 + j);
             const int tmp = cur; cur = nxt; nxt = tmp;
         }
 
@@ -658,7 +664,9 @@ __global__ void __launch_bounds__(MAXT, MINB) eval_team_kernel(EvalArgs a, TeamD
         if (nsp == 1) {
             team_combine<C, C>(smd, d, ncfg, recSQ, tid, nthreads);
             __syncthreads();
+            COS_PHASE_MARK(12);
             team_reduce<C>(CB, DB, ncfg, n, mask16, lvlT, tid, nthreads);
+            COS_PHASE_MARK(13);
             if (tid < ncfg) a.out[cfgbase + tid] = CB[red_elem<C>((NS >> (1 + kRedLB)) - 1, 15u, tid)];
         } else {
             team_combine<C, C / 2>(smd, d, ncfg, recSQ, tid, nthreads);

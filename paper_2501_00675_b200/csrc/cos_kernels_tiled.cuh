@@ -403,7 +403,7 @@ __device__ __forceinline__ void small_stages(const double* W, int n, double* z /
 namespace cosb {
 
 #ifdef COS_PHASE_TIMING
-__device__ unsigned long long g_phase_cycles[8];
+__device__ unsigned long long g_phase_cycles[32];
 #define COS_PHASE_MARK(k) do { __syncthreads(); if (threadIdx.x == 0) { const long long now__ = clock64(); \
     atomicAdd(&g_phase_cycles[k], (unsigned long long)(now__ - phase_t0__)); phase_t0__ = now__; } } while (0)
 #else
