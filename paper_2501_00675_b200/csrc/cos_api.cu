@@ -134,9 +134,9 @@ int do_build_G(cos_ctx* c, int n, long long batch, const int* xy, const double* 
     a.Tup = c->table[0]; a.Tdn = c->table[1];
     a.Lx = c->Lx; a.Ly = c->Ly; a.ntau = c->ntau; a.beta = c->beta; a.g_diag = g_diag;
     a.Gup = gup; a.Gdn = (gdn == gup) ? nullptr : gdn;
-    const long long total = batch * n * n;
-    long long blocks = (total + 255) / 256;
-    const long long cap = (long long)c->num_sms * 16;
+    const int per_cta = 256 / (n * n) > 0 ? 256 / (n * n) : 1;     // configurations per CTA pass (see the kernel)
+    long long blocks = (batch + per_cta - 1) / per_cta;
+    const long long cap = (long long)c->num_sms * 64;
     if (blocks > cap) blocks = cap;
     build_G_kernel<<<(unsigned)blocks, 256, 0, c->stream>>>(a);
     COS_CUDA(c, cudaGetLastError());

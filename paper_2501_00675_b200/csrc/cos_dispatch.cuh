@@ -93,12 +93,10 @@ inline PairChoice pair_choice(int n, int nsp)
     return {eval_pair_kernel<4, 576, 1, 8>, pair_dims<4>(n, nsp)};
 }
 
-inline bool has_fused_kernel(int n, int nsp, int smem_optin)
-{
-    if (uses_team(n)) return team_choice(n, nsp).d.smem_bytes <= (size_t)smem_optin;
-    if (uses_pair(n)) return pair_choice(n, nsp).d.smem_bytes <= (size_t)smem_optin;
-    return false;
-}
+// No evaluation kernel assembles G on the fly any more: a separate cos_build_G launch plus a cp.async prefetch of
+// the next team's matrices measured faster than the in-kernel gather (whose two dependent global round trips per
+// team sat on the critical path), and G costs 16 n^2 bytes per configuration of HBM traffic -- noise.
+inline bool has_fused_kernel(int, int, int) { return false; }
 
 using TiledKernel = void (*)(EvalArgs, TiledDims);
 inline TiledKernel tiled_kernel() { return eval_tiled_kernel<kTiledB, kTiledThreads, kTiledNA, kTiledJB, false>; }
@@ -131,13 +129,14 @@ inline cudaError_t dispatch_eval(const EvalArgs& a, cudaStream_t stream, int num
         const TeamChoice tc = team_choice(a.n, nsp);
         if (tc.d.smem_bytes <= (size_t)smem_optin) {
             int per_sm = 1;
-            cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, tc.fn, tc.d.threads, tc.d.smem_bytes);
+            const int block = tc.d.threads;
+            cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, tc.fn, block, tc.d.smem_bytes);
             if (e != cudaSuccess) return e;
             if (per_sm < 1) per_sm = 1;
             const long long teams = (a.batch * nsp + tc.d.C - 1) / tc.d.C;
             long long grid = (long long)num_sms * per_sm;
             if (grid > teams) grid = teams;
-            tc.fn<<<(unsigned)grid, tc.d.threads, tc.d.smem_bytes, stream>>>(a, tc.d);
+            tc.fn<<<(unsigned)grid, block, tc.d.smem_bytes, stream>>>(a, tc.d);
             *name = "eval_team_kernel";
             return cudaGetLastError();
         }

@@ -22,14 +22,14 @@ namespace cosb {
 // One thread per (b, i, j).  Table rows are L2 resident (1-8 MiB); two adjacent tau points per entry.
 // One entry G_s[b][i][j] (both species) of step a1; shared by build_G_kernel and the fused evaluation kernels so
 // that both produce bit-identical matrices.
-__device__ __forceinline__ void g0_entry(const BuildGArgs& a, long long b, int i, int j, double& gup, double& gdn)
+// Off-diagonal value from the coordinates of the two vertices (reading R8: 2-point lerp on the tau grid,
+// antiperiodic branch for dtau <= 0, R9).
+__device__ __forceinline__ void g0_value(const BuildGArgs& a, int xi, int yi, int xj, int yj, double ti, double tj,
+                                         double& gup, double& gdn)
 {
-    if (i == j) { gup = a.g_diag; gdn = a.g_diag; return; }
-    const int* pi = a.xy + (b * a.n + i) * 2;
-    const int* pj = a.xy + (b * a.n + j) * 2;
-    int dx = (pi[0] - pj[0]) % a.Lx; if (dx < 0) dx += a.Lx;
-    int dy = (pi[1] - pj[1]) % a.Ly; if (dy < 0) dy += a.Ly;
-    double dtau = a.tau[b * a.n + i] - a.tau[b * a.n + j];
+    int dx = (xi - xj) % a.Lx; if (dx < 0) dx += a.Lx;
+    int dy = (yi - yj) % a.Ly; if (dy < 0) dy += a.Ly;
+    double dtau = ti - tj;
     double sign = 1.0;
     if (dtau <= 0.0) { dtau = __dadd_rn(dtau, a.beta); sign = -1.0; }     // R9: dtau == 0 is 0-
     const double uu = __ddiv_rn(__dmul_rn(dtau, (double)(a.ntau - 1)), a.beta);
@@ -50,19 +50,27 @@ __device__ __forceinline__ void g0_entry(const BuildGArgs& a, long long b, int i
     }
 }
 
+__device__ __forceinline__ void g0_entry(const BuildGArgs& a, long long b, int i, int j, double& gup, double& gdn)
+{
+    if (i == j) { gup = a.g_diag; gdn = a.g_diag; return; }
+    const int* pi = a.xy + (b * a.n + i) * 2;
+    const int* pj = a.xy + (b * a.n + j) * 2;
+    g0_value(a, pi[0], pi[1], pj[0], pj[1], a.tau[b * a.n + i], a.tau[b * a.n + j], gup, gdn);
+}
+
+// One thread per (b, i, j); a CTA walks whole configurations so that the index arithmetic stays 32-bit.
 __global__ void __launch_bounds__(256) build_G_kernel(BuildGArgs a)
 {
-    const long long total = a.batch * a.n * a.n;
-    for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < total;
-         t += (long long)gridDim.x * blockDim.x) {
-        const int j = (int)(t % a.n);
-        const long long bi = t / a.n;
-        const int i = (int)(bi % a.n);
-        const long long b = bi / a.n;
+    const int nn = a.n * a.n;
+    const int per_cta = 256 / nn > 0 ? 256 / nn : 1;          // configurations per CTA pass (n <= 16: nn <= 256)
+    const int local = threadIdx.x / nn, e = threadIdx.x - local * nn;
+    if (local >= per_cta) return;
+    const int i = e / a.n, j = e - i * a.n;
+    for (long long b = (long long)blockIdx.x * per_cta + local; b < a.batch; b += (long long)gridDim.x * per_cta) {
         double gup, gdn;
         g0_entry(a, b, i, j, gup, gdn);
-        a.Gup[t] = gup;
-        if (a.Gdn) a.Gdn[t] = gdn;
+        a.Gup[b * nn + e] = gup;
+        if (a.Gdn) a.Gdn[b * nn + e] = gdn;
     }
 }
 

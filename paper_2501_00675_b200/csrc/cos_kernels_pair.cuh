@@ -62,6 +62,7 @@ struct PairDims {
     int red_rows;      // 2^(n-1-kRedLB) block rows of the reduction arrays
     int off_w, off_u, off_z, off_b0, off_b1;   // double offsets behind the tables
     int off_cb, off_db;                        // reduction arrays (alias the frontier buffers)
+    int off_stage;                             // staging buffer: G and u of the next team (cp.async)
     int tab_bytes;
     size_t smem_bytes;
 };
@@ -97,8 +98,9 @@ inline PairDims pair_dims(int n, int nsp)
     if (work < need) work = need;
     d.off_cb = d.off_b0;
     d.off_db = d.off_b0 + d.red_rows * 16 * d.ncfg;
+    d.off_stage = d.off_b0 + work;                        // staging: [C * n * n] G, [C * n] u
     d.tab_bytes = ((2 * 2 * (1 << (n - 1)) + 4 * 64 + 2 * d.zrec) + 15) & ~15;   // mask16, rank16, lvlT, lvlZ, recSQ
-    d.smem_bytes = (size_t)d.tab_bytes + sizeof(double) * (size_t)(d.off_b0 + work);
+    d.smem_bytes = (size_t)d.tab_bytes + sizeof(double) * (size_t)(d.off_stage + C * n * n + C * n);
     return d;
 }
 
@@ -338,43 +340,6 @@ __device__ __forceinline__ void pair_combine(double* smd, const PairDims& d, int
     }
 }
 
-// One team's W matrices into shared memory (a1 fused, or a load of materialised G), instance fastest; -u_a is
-// folded into the rows of species 0 when the species are distinct.  Entry e of instance gi, replica r at
-// e * 16 + r * C + gi.
-template <int C>
-__device__ __forceinline__ void pair_load_w(const EvalArgs& a, const PairDims& d, double* smd, long long inst0, int ninst,
-                                            int tid, int nthreads)
-{
-    using Lay = PairLayout<C>;
-    const int n = d.n, nsp = d.nsp;
-    for (int t = tid; t < C * n * n; t += nthreads) {
-        const int gi = t % C, e = t / C;
-        double val = 0.0;
-        if (gi < ninst) {
-            const long long b = (inst0 + gi) / nsp;
-            const int s = (int)((inst0 + gi) % nsp);
-            if (a.fused) {
-                double gu, gd;
-                g0_entry(a.bg, b, e / n, e % n, gu, gd);
-                val = s ? gd : gu;
-            } else {
-                val = (s == 0 ? a.Gup : a.Gdn)[b * n * n + e];
-            }
-            if (nsp == 2 && s == 0) val *= -(a.u ? a.u[b * n + e / n] : a.U);
-        }
-        double* w = smd + d.off_w + e * Lay::WE + gi;
-#pragma unroll
-        for (int r = 0; r < Lay::REP; ++r) w[r * C] = val;
-    }
-    if (nsp == 1) {     // un[v][cfg] = -u_v (aliased species only: w(S) is applied in the combine step)
-        const int NCt = C, ncfg = ninst;
-        for (int t = tid; t < NCt * n; t += nthreads) {
-            const int cg = t % NCt, v = t / NCt;
-            smd[d.off_u + v * NCt + cg] = (cg < ncfg) ? -(a.u ? a.u[(inst0 + cg) * n + v] : a.U) : 0.0;
-        }
-    }
-}
-
 template <int C, int MAXT, int MINB, int MAXNC>
 __global__ void __launch_bounds__(MAXT, MINB) eval_pair_kernel(EvalArgs a, PairDims d)
 {
@@ -420,14 +385,24 @@ __global__ void __launch_bounds__(MAXT, MINB) eval_pair_kernel(EvalArgs a, PairD
 
     const long long total_inst = a.batch * nsp;
     const long long nteams = (total_inst + C - 1) / C;
+    double* stage = smd + d.off_stage;
+    if ((long long)blockIdx.x < nteams) {
+        const long long nx0 = (long long)blockIdx.x * C;
+        team_prefetch_inputs<C>(a, n, nsp, stage, nx0, (int)min((long long)C, total_inst - nx0), tid, nthreads);
+    }
     for (long long team = blockIdx.x; team < nteams; team += gridDim.x) {
         const long long inst0 = team * C;
         const int ninst = (int)min((long long)C, total_inst - inst0);
         const int ncfg = ninst / nsp;
         const long long cfgbase = inst0 / nsp;
+        cp_async_wait_all();
         __syncthreads();
-        pair_load_w<C>(a, d, smd, inst0, ninst, tid, nthreads);
+        team_unpack_inputs<C, REP>(a, n, nsp, stage, smd + d.off_w, smd + d.off_u, ninst, tid, nthreads);
         __syncthreads();
+        if (team + gridDim.x < nteams) {
+            const long long nx0 = (team + gridDim.x) * C;
+            team_prefetch_inputs<C>(a, n, nsp, stage, nx0, (int)min((long long)C, total_inst - nx0), tid, nthreads);
+        }
         COS_PHASE_MARK(0);
         if (tid < ninst) pair_small_stages<C>(smd + d.off_w + tid, n, smd + d.off_z + tid * 4);
         __syncthreads();

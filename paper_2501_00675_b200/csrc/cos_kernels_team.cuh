@@ -77,6 +77,7 @@ struct TeamDims {
     int red_rows;      // 2^(n-1-kRedLB) block rows of the reduction arrays
     int off_w, off_u, off_z, off_b0, off_b1;   // double offsets behind the tables
     int off_cb, off_db;                        // reduction arrays (alias the frontier buffers)
+    int off_stage;                             // staging buffer: G and u of the next team (cp.async)
     int tab_bytes;
     size_t smem_bytes;
 };
@@ -121,8 +122,9 @@ inline TeamDims team_dims(int n, int nsp)
     d.off_b1 = d.off_b0 + maxrec * L::REC;
     d.off_cb = d.off_b0;
     d.off_db = d.off_b0 + d.red_rows * 16 * d.ncfg;
+    d.off_stage = d.off_b0 + work;                        // staging: [C * n * n] G, [C * n] u
     d.tab_bytes = ((2 * 2 * (1 << (n - 1)) + 4 * 64 + 2 * d.zrec) + 15) & ~15;   // mask16, rank16, lvlT, lvlZ, recSQ
-    d.smem_bytes = (size_t)d.tab_bytes + sizeof(double) * (size_t)(d.off_b0 + work);
+    d.smem_bytes = (size_t)d.tab_bytes + sizeof(double) * (size_t)(d.off_stage + C * n * n + C * n);
     return d;
 }
 
@@ -324,6 +326,15 @@ __device__ __forceinline__ void team_small_stages(const double* Wl, int n, doubl
 //   convolution over lo (81 FMAs on 32 loaded values).  The 2^|S_hi| terms of one output are split over 2^s
 //   lanes of one warp (lane bit k owns the k-th lowest vertex of S_hi), partial blocks are summed by a
 //   recursive-halving shuffle exchange, and the diagonal block (T_hi = S_hi) is solved in registers.
+// Block barrier of the team / pair kernels (every thread of the CTA is a compute thread).
+__device__ __forceinline__ void team_sync(int) { __syncthreads(); }
+#ifdef COS_PHASE_TIMING
+#define COS_PHASE_MARK_T(k, nthr) do { team_sync(nthr); if (threadIdx.x == 0) { const long long now__ = clock64(); \
+    atomicAdd(&g_phase_cycles[k], (unsigned long long)(now__ - phase_t0__)); phase_t0__ = now__; } } while (0)
+#else
+#define COS_PHASE_MARK_T(k, nthr) do { } while (0)
+#endif
+
 template <int NC> struct RedLayout {
     static constexpr int ROW = 16 * NC;
     static constexpr int PSTR = 2 * NC;
@@ -482,7 +493,7 @@ __device__ __forceinline__ void team_reduce(double* CB, const double* DB, int nc
                     *reinterpret_cast<double2*>(row + (p ^ sw) * R::PSTR) = make_double2(acc[2 * p], acc[2 * p + 1]);
             }
         }
-        __syncthreads();
+        team_sync(nthreads);
     }
 }
 
@@ -537,6 +548,65 @@ __device__ __forceinline__ void team_combine(double* smd, const TeamDims& d, int
     }
 }
 
+// ---- inputs of one team: G (materialised by cos_build_G or by the caller) and the couplings ----
+// The matrices of the NEXT team are fetched with cp.async into a staging buffer while the current team is being
+// evaluated (stage[gi * n*n + e], coalesced rows of G; then u[cg * n + v] when per-vertex couplings are given), and
+// unpacked into the replicated, instance-interleaved W at the start of the team:
+//   W[e * (REP * C) + r * C + gi],  -u_a folded into the rows of species 0 when the species are distinct,
+//   un[v * NCt + cg] = -u_v otherwise (w(S) is then applied in the combine step).
+__device__ __forceinline__ void cp_async8(void* smem_dst, const void* gsrc)
+{
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((unsigned)__cvta_generic_to_shared(smem_dst)), "l"(gsrc)
+                 : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+
+template <int C>
+__device__ __forceinline__ void team_prefetch_inputs(const EvalArgs& a, int n, int nsp, double* stage, long long inst0,
+                                                     int ninst, int tid, int nthreads)
+{
+    const int nn = n * n;
+    for (int t = tid; t < ninst * nn; t += nthreads) {
+        const int gi = t / nn, e = t - gi * nn;
+        const long long b = (inst0 + gi) >> (nsp - 1);            // nsp is 1 or 2
+        const int s = (int)((inst0 + gi) & (nsp - 1));
+        cp_async8(stage + t, (s == 0 ? a.Gup : a.Gdn) + b * nn + e);
+    }
+    if (a.u) {
+        const long long cfg0 = inst0 >> (nsp - 1);
+        const int ncfg = ninst >> (nsp - 1);
+        for (int t = tid; t < ncfg * n; t += nthreads) cp_async8(stage + C * nn + t, a.u + cfg0 * n + t);
+    }
+    cp_async_commit();
+}
+
+template <int C, int REP>
+__device__ __forceinline__ void team_unpack_inputs(const EvalArgs& a, int n, int nsp, const double* stage, double* Wd,
+                                                   double* un, int ninst, int tid, int nthreads)
+{
+    constexpr int WE = REP * C;
+    const int nn = n * n;
+    const int NCt = C / nsp, ncfg = ninst / nsp;
+    const double* su = stage + C * nn;
+    for (int t = tid; t < C * nn; t += nthreads) {
+        const int gi = t % C, e = t / C;
+        double val = 0.0;
+        if (gi < ninst) {
+            val = stage[gi * nn + e];
+            if (nsp == 2 && (gi & 1) == 0) val *= -(a.u ? su[(gi >> 1) * n + e / n] : a.U);
+        }
+        double* w = Wd + e * WE + gi;
+#pragma unroll
+        for (int r = 0; r < REP; ++r) w[r * C] = val;
+    }
+    if (nsp == 1)
+        for (int t = tid; t < NCt * n; t += nthreads) {
+            const int cg = t % NCt, v = t / NCt;
+            un[t] = (cg < ncfg) ? -(a.u ? su[cg * n + v] : a.U) : 0.0;
+        }
+}
+
 template <int C, int MAXT, int MINB>
 __global__ void __launch_bounds__(MAXT, MINB) eval_team_kernel(EvalArgs a, TeamDims d)
 {
@@ -555,6 +625,9 @@ __global__ void __launch_bounds__(MAXT, MINB) eval_team_kernel(EvalArgs a, TeamD
     const int tid = threadIdx.x, nthreads = blockDim.x;
     const int n = d.n, qmax = d.qmax, nsp = d.nsp;
     const unsigned NS = 1u << n;
+    const long long total_inst = a.batch * nsp;
+    const long long nteams = (total_inst + C - 1) / C;
+
     const int g = tid % C;                       // instance of this thread
     const int slot = tid / C;                    // pattern slot
     const int rep = slot % REP;                  // W replica read by this thread
@@ -568,7 +641,7 @@ __global__ void __launch_bounds__(MAXT, MINB) eval_team_kernel(EvalArgs a, TeamD
         run = 0;
         for (int j = 0; j <= qmax + 1; ++j) { lvlZ[j] = run; run += kBinom.c[qmax][j]; }
     }
-    __syncthreads();
+    team_sync(nthreads);
     for (unsigned mk = tid; mk < (1u << (n - 1)); mk += nthreads) {
         int rk = 0, i = 0;
         unsigned m = mk;
@@ -577,50 +650,30 @@ __global__ void __launch_bounds__(MAXT, MINB) eval_team_kernel(EvalArgs a, TeamD
         mask16[lvlT[i] + rk] = (uint16_t)mk;
         if (mk < (1u << qmax)) recSQ[lvlZ[i] + rk] = (uint16_t)mk;
     }
-    __syncthreads();
 
-    const long long total_inst = a.batch * nsp;
-    const long long nteams = (total_inst + C - 1) / C;
+    double* stage = smd + d.off_stage;
+    if ((long long)blockIdx.x < nteams) {
+        const long long nx0 = (long long)blockIdx.x * C;
+        team_prefetch_inputs<C>(a, n, nsp, stage, nx0, (int)min((long long)C, total_inst - nx0), tid, nthreads);
+    }
     for (long long team = blockIdx.x; team < nteams; team += gridDim.x) {
         const long long inst0 = team * C;
         const int ninst = (int)min((long long)C, total_inst - inst0);
         const int ncfg = ninst / nsp;
         const int NCt = C / nsp;                 // configuration slots of a team
         const long long cfgbase = inst0 / nsp;
+        cp_async_wait_all();
         __syncthreads();
-        // ---- a1 (fused) / load: W of every instance, instance fastest; -u_a folded into the rows of species 0
-        //      when the species are distinct.  Replica r of entry e lives at e*WE + r*C + g. ----
-        for (int t = tid; t < C * n * n; t += nthreads) {
-            const int gi = t % C, e = t / C;
-            double val = 0.0;
-            if (gi < ninst) {
-                const long long b = (inst0 + gi) / nsp;
-                const int s = (int)((inst0 + gi) % nsp);
-                if (a.fused) {
-                    double gu, gd;
-                    g0_entry(a.bg, b, e / n, e % n, gu, gd);
-                    val = s ? gd : gu;
-                } else {
-                    val = (s == 0 ? a.Gup : a.Gdn)[b * n * n + e];
-                }
-                if (nsp == 2 && s == 0) val *= -(a.u ? a.u[b * n + e / n] : a.U);
-            }
-            double* w = smd + d.off_w + e * WE + gi;
-#pragma unroll
-            for (int r = 0; r < REP; ++r) w[((r + e) % REP) * C] = val;
-        }
-        // un[v][cfg] = -u_v (aliased species only: w(S) is applied in the combine step)
-        if (nsp == 1) {
-            for (int t = tid; t < NCt * n; t += nthreads) {
-                const int cg = t % NCt, v = t / NCt;
-                smd[d.off_u + v * NCt + cg] = (cg < ncfg) ? -(a.u ? a.u[(cfgbase + cg) * n + v] : a.U) : 0.0;
-            }
-        }
+        team_unpack_inputs<C, REP>(a, n, nsp, stage, smd + d.off_w, smd + d.off_u, ninst, tid, nthreads);
         __syncthreads();
-        COS_PHASE_MARK(0);
+        if (team + gridDim.x < nteams) {
+            const long long nx0 = (team + gridDim.x) * C;
+            team_prefetch_inputs<C>(a, n, nsp, stage, nx0, (int)min((long long)C, total_inst - nx0), tid, nthreads);
+        }
+        COS_PHASE_MARK_T(0, nthreads);
         if (tid < ninst) team_small_stages<C>(smd + d.off_w + tid, n, smd + d.off_z + tid * 2);
-        __syncthreads();
-        COS_PHASE_MARK(1);
+        team_sync(nthreads);
+        COS_PHASE_MARK_T(1, nthreads);
 
         // ---- a2: all stages together, level j = |S_Q| - 1 ----
         TeamLevel L;
@@ -638,8 +691,8 @@ __global__ void __launch_bounds__(MAXT, MINB) eval_team_kernel(EvalArgs a, TeamD
                 const bool active = (x < L.cnt) && (g < ninst);
                 team_dispatch_item<C>(L, active ? masks[x] : 1u, x, sm, Wl, active);
             }
-            __syncthreads();
-            COS_PHASE_MARK(2 + j);
+            team_sync(nthreads);
+            COS_PHASE_MARK_T(2 + j, nthreads);
             const int tmp = cur; cur = nxt; nxt = tmp;
         }
 
@@ -663,15 +716,17 @@ __global__ void __launch_bounds__(MAXT, MINB) eval_team_kernel(EvalArgs a, TeamD
         const double* DB = smd + d.off_db;
         if (nsp == 1) {
             team_combine<C, C>(smd, d, ncfg, recSQ, tid, nthreads);
-            __syncthreads();
-            COS_PHASE_MARK(12);
+            team_sync(nthreads);
+            COS_PHASE_MARK_T(12, nthreads);
             team_reduce<C>(CB, DB, ncfg, n, mask16, lvlT, tid, nthreads);
-            COS_PHASE_MARK(13);
+            COS_PHASE_MARK_T(13, nthreads);
             if (tid < ncfg) a.out[cfgbase + tid] = CB[red_elem<C>((NS >> (1 + kRedLB)) - 1, 15u, tid)];
         } else {
             team_combine<C, C / 2>(smd, d, ncfg, recSQ, tid, nthreads);
-            __syncthreads();
+            team_sync(nthreads);
+            COS_PHASE_MARK_T(12, nthreads);
             team_reduce<C / 2>(CB, DB, ncfg, n, mask16, lvlT, tid, nthreads);
+            COS_PHASE_MARK_T(13, nthreads);
             if (tid < ncfg) a.out[cfgbase + tid] = CB[red_elem<C / 2>((NS >> (1 + kRedLB)) - 1, 15u, tid)];
         }
     }
