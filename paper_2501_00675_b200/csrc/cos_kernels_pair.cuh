@@ -443,7 +443,7 @@ __global__ void __launch_bounds__(MAXT, MINB) eval_pair_kernel(EvalArgs a, PairD
 
         // ---- a3: combine, a4: connected reduction, a5: C'[full] ----
         double* CB = smd + d.off_cb;
-        const double* DB = smd + d.off_db;
+        double* DB = smd + d.off_db;
         if (nsp == 1) {
             pair_combine<C, C>(smd, d, ncfg, recSQ, tid, nthreads);
             __syncthreads();

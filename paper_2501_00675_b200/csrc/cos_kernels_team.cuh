@@ -78,6 +78,7 @@ struct TeamDims {
     int off_w, off_u, off_z, off_b0, off_b1;   // double offsets behind the tables
     int off_cb, off_db;                        // reduction arrays (alias the frontier buffers)
     int off_stage;                             // staging buffer: G and u of the next team (cp.async)
+    int dsc_off;                               // byte offset of the item descriptors inside the table area
     int tab_bytes;
     size_t smem_bytes;
 };
@@ -123,7 +124,8 @@ inline TeamDims team_dims(int n, int nsp)
     d.off_cb = d.off_b0;
     d.off_db = d.off_b0 + d.red_rows * 16 * d.ncfg;
     d.off_stage = d.off_b0 + work;                        // staging: [C * n * n] G, [C * n] u
-    d.tab_bytes = ((2 * 2 * (1 << (n - 1)) + 4 * 64 + 2 * d.zrec) + 15) & ~15;   // mask16, rank16, lvlT, lvlZ, recSQ
+    d.dsc_off = ((2 * 2 * (1 << (n - 1)) + 4 * 64 + 2 * d.zrec) + 31) & ~31;     // mask16, rank16, lvlT, lvlZ, recSQ
+    d.tab_bytes = d.dsc_off + 32 * d.zrec;                                        // + one 32-byte descriptor per pattern
     d.smem_bytes = (size_t)d.tab_bytes + sizeof(double) * (size_t)(d.off_stage + C * n * n + C * n);
     return d;
 }
@@ -154,38 +156,68 @@ __device__ __forceinline__ void team_load_rec(const RecPtr<C>& r, double (&a)[kT
 // N = q - j Q-targets are accumulated in registers together with the close (column h) and the T-targets.
 // N is the number of Q-targets of the widest item of the WARP (warp-uniform, so the dispatch never diverges); an
 // item with fewer targets (Nown < N) pads with dummy targets that read a valid W column and are never stored.
+// Item descriptor of pattern S_Q (8 words, indexed by the Z record number of S_Q), built once per CTA: everything
+// an item needs to know about the graph, so that its prologue is one wide load instead of a chain of bit tricks
+// and rank look-ups (the measured critical path of a level was that chain, not the arithmetic).
+//   w0: S_Q | Z record of S_Q \ {top} << 16        w1..w3: record numbers of the (at most 6) Q-targets, 16 bits each
+//   w4: column vertices of the Q-targets, 4 bits each (padding: h); bits 24..27: h; bits 28..31: number of Q-targets
+//   w5: source vertices (elements of S_Q \ {top}, ascending, + 3), 4 bits each
+__device__ __forceinline__ void team_build_descriptor(uint32_t* dsc, unsigned SQ, int qmax, const int* lvlZ,
+                                                      const uint16_t* rank16)
+{
+    constexpr int B = kTeamB;
+    const int j = __popc(SQ) - 1;
+    const int q = 31 - __clz((int)SQ);
+    const unsigned RQ = SQ ^ (1u << q);
+    const int h = q + B;
+    const int cnt_next = kBinom.c[qmax][j + 2];
+    uint32_t w[8] = {0, 0xffffffffu, 0xffffffffu, 0xffffffffu, 0, 0, 0, 0};
+    w[0] = SQ | ((uint32_t)(lvlZ[j] + rank16[RQ]) << 16);
+    unsigned absent = ~RQ & ((1u << q) - 1u);
+    int k = 0;
+    uint32_t cols = 0;
+    for (; absent && k < kTeamMaxTargets; ++k) {
+        const int dd = __ffs(absent) - 1;
+        absent &= absent - 1;
+        const uint32_t orec = (uint32_t)(__popc(RQ & ((1u << dd) - 1u)) * cnt_next + rank16[SQ | (1u << dd)]);
+        const int wi = 1 + (k >> 1), sh = (k & 1) * 16;
+        w[wi] = (w[wi] & ~(0xffffu << sh)) | (orec << sh);
+        cols |= (uint32_t)(dd + B) << (4 * k);
+    }
+    const int nown = k;
+    for (; k < kTeamMaxTargets; ++k) cols |= (uint32_t)h << (4 * k);
+    w[4] = cols | ((uint32_t)h << 24) | ((uint32_t)nown << 28);
+    unsigned m = RQ;
+    for (int i = 0; m; ++i) { const int v = __ffs(m) - 1 + B; m &= m - 1; w[5] |= (uint32_t)v << (4 * i); }
+#pragma unroll
+    for (int i = 0; i < 8; ++i) dsc[i] = w[i];
+}
+
 template <int C, int N>
-__device__ __forceinline__ void team_item(const TeamLevel& L, unsigned SQ, int x, double* sm, const double* Wl)
+__device__ __forceinline__ void team_item(const TeamLevel& L, const uint32_t* dsc, int x, double* sm, const double* Wl)
 {
     using Lay = TeamLayout<C>;
     constexpr int WE = Lay::WE, NT = kTeamNT, B = kTeamB;
     const int n = L.n;
-    const int q = 31 - __clz((int)SQ);
-    const unsigned RQ = SQ ^ (1u << q);
-    const int h = q + B;
+    const uint4 d0 = *reinterpret_cast<const uint4*>(dsc);
+    const uint2 d1 = *reinterpret_cast<const uint2*>(dsc + 4);
+    const int zrec = (int)(d0.x >> 16);
+    const int h = (int)((d1.x >> 24) & 15u);
     int colo[N + 1];                  // W column offset of target k; the last one is the close column h
-    int orec[N > 0 ? N : 1];          // record number of target k in the next buffer
-    {
-        unsigned absent = ~RQ & ((1u << q) - 1u);
+    int orec[N > 0 ? N : 1];          // record number of target k in the next buffer (0xffff: dummy target)
 #pragma unroll
-        for (int k = 0; k < N; ++k) {
-            if (absent) {
-                const int d = __ffs(absent) - 1;
-                absent &= absent - 1;
-                colo[k] = (d + B) * WE;
-                orec[k] = __popc(RQ & ((1u << d) - 1u)) * L.cnt_next + L.rank16[SQ | (1u << d)];
-            } else {
-                colo[k] = h * WE;      // dummy target
-                orec[k] = -1;
-            }
-        }
-        colo[N] = h * WE;
+    for (int k = 0; k < N; ++k) {
+        colo[k] = (int)((d1.x >> (4 * k)) & 15u) * WE;
+        const uint32_t pr = (k >> 1) == 0 ? d0.y : ((k >> 1) == 1 ? d0.z : d0.w);
+        orec[k] = (int)((k & 1) ? (pr >> 16) : (pr & 0xffffu));
     }
+    colo[N] = h * WE;
+    unsigned srcs = d1.y;
     const int rowstride = n * WE;
     double acc[NT][N + 1], accT[NT][B];
     // ---- phase 1a: the start node (S, h) = Z[S \ {h}] ("top node", one per stage) ----
     {
-        const RecPtr<C> zp(sm + L.off_z, L.lvlZ_j + L.rank16[RQ]);
+        const RecPtr<C> zp(sm + L.off_z, zrec);
         double a[NT];
         team_load_rec<C>(zp, a);
         const double* row = Wl + h * rowstride;
@@ -204,11 +236,10 @@ __device__ __forceinline__ void team_item(const TeamLevel& L, unsigned SQ, int x
     }
     // ---- phase 1b: sources in Q, streamed from the level buffer ----
     {
-        unsigned m = RQ;
         int rec = x;
         for (int i = 0; i < L.j; ++i) {
-            const int v = __ffs(m) - 1 + B;
-            m &= m - 1;
+            const int v = (int)(srcs & 15u);
+            srcs >>= 4;
             const RecPtr<C> rp(sm + L.off_cur, rec);
             rec += L.cnt;
             const double* row = Wl + v * rowstride;
@@ -257,7 +288,7 @@ __device__ __forceinline__ void team_item(const TeamLevel& L, unsigned SQ, int x
     // ---- outputs: next-level records, and Z[(SQ, R_T)] = -close (one -1 per closed fermion loop) ----
 #pragma unroll
     for (int k = 0; k < N; ++k) {
-        if (orec[k] < 0) continue;
+        if (orec[k] == 0xffff) continue;
         const RecPtr<C> o(sm + L.off_nxt, orec[k]);
 #pragma unroll
         for (int p = 0; p < 4; ++p)
@@ -272,21 +303,21 @@ __device__ __forceinline__ void team_item(const TeamLevel& L, unsigned SQ, int x
 }
 
 template <int C>
-__device__ __forceinline__ void team_dispatch_item(const TeamLevel& L, unsigned SQ, int x, double* sm, const double* Wl,
-                                                   bool active)
+__device__ __forceinline__ void team_dispatch_item(const TeamLevel& L, const uint32_t* dsc, int x, double* sm,
+                                                   const double* Wl, bool active)
 {
     // warp-uniform target count: the widest item of the warp (all 32 lanes call this)
-    const int Nown = active ? (31 - __clz((int)SQ)) - L.j : 0;
+    const int Nown = active ? (int)(dsc[4] >> 28) : 0;
     const int N = __reduce_max_sync(0xffffffffu, Nown);
     if (!active) return;
     switch (N) {
-        case 0: team_item<C, 0>(L, SQ, x, sm, Wl); break;
-        case 1: team_item<C, 1>(L, SQ, x, sm, Wl); break;
-        case 2: team_item<C, 2>(L, SQ, x, sm, Wl); break;
-        case 3: team_item<C, 3>(L, SQ, x, sm, Wl); break;
-        case 4: team_item<C, 4>(L, SQ, x, sm, Wl); break;
-        case 5: team_item<C, 5>(L, SQ, x, sm, Wl); break;
-        default: team_item<C, 6>(L, SQ, x, sm, Wl); break;
+        case 0: team_item<C, 0>(L, dsc, x, sm, Wl); break;
+        case 1: team_item<C, 1>(L, dsc, x, sm, Wl); break;
+        case 2: team_item<C, 2>(L, dsc, x, sm, Wl); break;
+        case 3: team_item<C, 3>(L, dsc, x, sm, Wl); break;
+        case 4: team_item<C, 4>(L, dsc, x, sm, Wl); break;
+        case 5: team_item<C, 5>(L, dsc, x, sm, Wl); break;
+        default: team_item<C, 6>(L, dsc, x, sm, Wl); break;
     }
 }
 
@@ -372,13 +403,56 @@ __device__ __forceinline__ void red_load_block(const double* arr, unsigned hi, i
 }
 
 template <int NC>
-__device__ __forceinline__ void team_reduce(double* CB, const double* DB, int ncfg, int n, const uint16_t* mask16,
+__device__ __forceinline__ void team_reduce(double* CB, double* DB, int ncfg, int n, const uint16_t* mask16,
                                             const int* lvlT, int tid, int nthreads)
 {
     using R = RedLayout<NC>;
     const int hb = n - 1 - kRedLB;
     const int cg = tid % NC, slot = tid / NC, slots = nthreads / NC;
-    for (int l = 0; l <= hb; ++l) {
+    // ---- make the diagonal block the identity: with g = (D1[hi = {}])^-1 (subset-convolution inverse over lo),
+    //      C' = D0 / D1 = (D0 * g) / (D1 * g) and (D1 * g)[hi = {}] = delta, so that C'[S_hi] needs no triangular
+    //      solve of its own -- the 65 dependent FMAs per output row leave the critical path of every level.
+    //      Cost: one lo-convolution per row of both arrays, all rows in parallel. ----
+    if (slot == 0 && cg < ncfg) {
+        double e[16], gi[16];
+        red_load_block<NC>(DB, 0u, cg, e);
+        gi[0] = 1.0;                                      // D[{}] = 1
+#pragma unroll
+        for (int lo = 1; lo < 16; ++lo) {
+            double v = 0.0;
+#pragma unroll
+            for (int T = 0; T < 16; ++T)
+                if ((T & ~lo) == 0 && T != lo) v = fma(-gi[T], e[lo ^ T], v);
+            gi[lo] = v;
+        }
+        double* row = DB + cg * 2;
+#pragma unroll
+        for (int p = 0; p < 8; ++p) *reinterpret_cast<double2*>(row + p * R::PSTR) = make_double2(gi[2 * p], gi[2 * p + 1]);   // row 0: no swizzle
+    }
+    team_sync(nthreads);
+    {
+        const int rows = 1 << hb;
+        if (cg < ncfg) {
+            double gi[16];
+            red_load_block<NC>(DB, 0u, cg, gi);
+            for (int task = slot; task < 2 * rows - 1; task += slots) {
+                double* arr = task < rows ? CB : DB;
+                const unsigned hi = (unsigned)(task < rows ? task : task - rows + 1);
+                double v[16], o[16];
+                red_load_block<NC>(arr, hi, cg, v);
+#pragma unroll
+                for (int t = 0; t < 16; ++t) o[t] = 0.0;
+                leaf_conv(v, gi, o);
+                double* row = arr + (int)hi * R::ROW + cg * 2;
+                const int sw = red_swz<NC>(hi);
+#pragma unroll
+                for (int p = 0; p < 8; ++p)
+                    *reinterpret_cast<double2*>(row + (p ^ sw) * R::PSTR) = make_double2(o[2 * p], o[2 * p + 1]);
+            }
+        }
+    }
+    team_sync(nthreads);
+    for (int l = 1; l <= hb; ++l) {
         const int outputs = kBinom.c[hb][l];
         int s = l < R::SMAX ? l : R::SMAX;
         while (s > 0 && (outputs << s) > slots) --s;
@@ -417,8 +491,14 @@ __device__ __forceinline__ void team_reduce(double* CB, const double* DB, int nc
             double* blk = CB;     // element lo at blk[red_elem(S, lo, cg)]
             if (s == 0) {
                 if (active) {
+                    double* row = CB + (int)S * R::ROW + cg * 2;
+                    const int sw = red_swz<NC>(S);
 #pragma unroll
-                    for (int t = 0; t < 16; ++t) acc[t] = blk[red_elem<NC>(S, t, cg)] - acc[t];
+                    for (int p = 0; p < 8; ++p) {
+                        double2* q2 = reinterpret_cast<double2*>(row + (p ^ sw) * R::PSTR);
+                        const double2 d0 = *q2;
+                        *q2 = make_double2(d0.x - acc[2 * p], d0.y - acc[2 * p + 1]);
+                    }
                 }
             } else {
                 double r8[8];
@@ -471,26 +551,6 @@ __device__ __forceinline__ void team_reduce(double* CB, const double* DB, int nc
                         }
                     }
                 }
-                __syncwarp();
-                if (active && c == 0) red_load_block<NC>(CB, S, cg, acc);
-            }
-            // ---- diagonal block: x[lo] = pre[lo] - sum_{T proper subset of lo} x[T] e[lo ^ T], e = D1[hi = {}] ----
-            if (active && c == 0) {
-                double e[16];
-                red_load_block<NC>(DB, 0u, cg, e);
-#pragma unroll
-                for (int lo = 1; lo < 16; ++lo) {
-                    double v = acc[lo];
-#pragma unroll
-                    for (int T = 0; T < 16; ++T)
-                        if ((T & ~lo) == 0 && T != lo) v = fma(-acc[T], e[lo ^ T], v);
-                    acc[lo] = v;
-                }
-                double* row = CB + (int)S * R::ROW + cg * 2;
-                const int sw = red_swz<NC>(S);
-#pragma unroll
-                for (int p = 0; p < 8; ++p)
-                    *reinterpret_cast<double2*>(row + (p ^ sw) * R::PSTR) = make_double2(acc[2 * p], acc[2 * p + 1]);
             }
         }
         team_sync(nthreads);
@@ -650,6 +710,9 @@ __global__ void __launch_bounds__(MAXT, MINB) eval_team_kernel(EvalArgs a, TeamD
         mask16[lvlT[i] + rk] = (uint16_t)mk;
         if (mk < (1u << qmax)) recSQ[lvlZ[i] + rk] = (uint16_t)mk;
     }
+    __syncthreads();
+    uint32_t* dtab = reinterpret_cast<uint32_t*>(smem_raw + d.dsc_off);
+    for (int r = 1 + tid; r < (1 << qmax); r += nthreads) team_build_descriptor(dtab + r * 8, recSQ[r], qmax, lvlZ, rank16);
 
     double* stage = smd + d.off_stage;
     if ((long long)blockIdx.x < nteams) {
@@ -685,11 +748,10 @@ __global__ void __launch_bounds__(MAXT, MINB) eval_team_kernel(EvalArgs a, TeamD
             L.cnt_next = kBinom.c[qmax][j + 2];
             L.lvlZ_j = lvlZ[j]; L.lvlZ_j1 = lvlZ[j + 1];
             L.off_cur = cur; L.off_nxt = nxt;
-            const uint16_t* masks = mask16 + lvlT[j + 1];
             for (int x0 = 0; x0 < L.cnt; x0 += d.pslots) {
                 const int x = x0 + slot;
                 const bool active = (x < L.cnt) && (g < ninst);
-                team_dispatch_item<C>(L, active ? masks[x] : 1u, x, sm, Wl, active);
+                team_dispatch_item<C>(L, dtab + (L.lvlZ_j1 + (active ? x : 0)) * 8, x, sm, Wl, active);
             }
             team_sync(nthreads);
             COS_PHASE_MARK_T(2 + j, nthreads);
@@ -713,7 +775,7 @@ __global__ void __launch_bounds__(MAXT, MINB) eval_team_kernel(EvalArgs a, TeamD
 
         // ---- a3: combine, a4: connected reduction, a5: C'[full] ----
         double* CB = smd + d.off_cb;
-        const double* DB = smd + d.off_db;
+        double* DB = smd + d.off_db;
         if (nsp == 1) {
             team_combine<C, C>(smd, d, ncfg, recSQ, tid, nthreads);
             team_sync(nthreads);
