@@ -81,7 +81,7 @@ inline TeamChoice team_choice(int n, int nsp)
 }
 
 // ---- pair kernel (orders 11..12): the team mapping with every item split over a lane pair ----
-constexpr int kPairMinN = 11, kPairMaxN = 12;
+constexpr int kPairMinN = 11, kPairMaxN = 13;
 using PairKernel = void (*)(EvalArgs, PairDims);
 struct PairChoice { PairKernel fn; PairDims d; };
 inline bool uses_pair(int n) { return n >= kPairMinN && n <= kPairMaxN; }
@@ -89,6 +89,7 @@ inline bool uses_pair(int n) { return n >= kPairMinN && n <= kPairMaxN; }
 inline bool has_fused_kernel(int n, int nsp, int smem_optin);
 inline PairChoice pair_choice(int n, int nsp)
 {
+    if (n == 13) return {eval_pair_kernel<1, 512, 1, 10>, pair_dims<1>(n, 1)};   // one species only (see dispatch_eval)
     if (n == 12) return {eval_pair_kernel<2, 512, 1, 9>, pair_dims<2>(n, nsp)};
     return {eval_pair_kernel<4, 576, 1, 8>, pair_dims<4>(n, nsp)};
 }
@@ -143,7 +144,7 @@ inline cudaError_t dispatch_eval(const EvalArgs& a, cudaStream_t stream, int num
     }
     if (uses_pair(a.n)) {
         const PairChoice tc = pair_choice(a.n, nsp);
-        if (tc.d.smem_bytes <= (size_t)smem_optin) {
+        if (tc.d.smem_bytes <= (size_t)smem_optin && tc.d.C >= nsp) {
             int per_sm = 1;
             cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, tc.fn, tc.d.threads, tc.d.smem_bytes);
             if (e != cudaSuccess) return e;

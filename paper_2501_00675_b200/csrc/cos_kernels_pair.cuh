@@ -34,12 +34,14 @@ constexpr int kPairB = 3;            // |T|
 constexpr int kPairMaxCols = 9;      // Q-targets + close held in registers (order 12: at most 8 + 1)
 
 template <int C> struct PairLayout {
-    static_assert(C == 2 || C == 4 || C == 8 || C == 16, "instances per team");
-    static constexpr int REP = 16 / C;           // W replicas: the 16 pairs of a warp read 16 distinct banks
-    static constexpr int WE = 16;                // doubles per W entry (REP * C)
+    static_assert(C == 1 || C == 2 || C == 4 || C == 8 || C == 16, "instances per team");
+    static constexpr int REP = C == 1 ? 4 : 16 / C;   // W replicas: the 16 pairs of a warp read distinct banks (C = 1: 4
+                                                      // replicas, some two-way conflicts, to stay inside shared memory)
+    static constexpr int WE = REP * C;           // doubles per W entry
     static constexpr int CH = 4 * C;             // doubles per record chunk
     static constexpr int REC = 8 * C;            // doubles per node record
-    static constexpr int SWZ = (C == 2) ? 1 : 0; // chunk swizzle by record parity
+    static constexpr int SWZ = (C <= 2) ? 1 : 0; // chunk swizzle by a record-number bit (C <= 2)
+    static constexpr int SWZSH = (C == 1) ? 1 : 0;   // which bit: records x, x+2 collide for C = 1, x, x+1 for C = 2
     static constexpr int PW = 16 / C;            // patterns per warp
 };
 
@@ -48,7 +50,7 @@ template <int C>
 __device__ __forceinline__ int pair_chunk(int rec, int p)
 {
     using L = PairLayout<C>;
-    return rec * L::REC + (L::SWZ ? ((p ^ rec) & 1) : p) * L::CH;
+    return rec * L::REC + (L::SWZ ? ((p ^ (rec >> L::SWZSH)) & 1) : p) * L::CH;
 }
 
 struct PairDims {
@@ -99,7 +101,7 @@ inline PairDims pair_dims(int n, int nsp)
     d.off_cb = d.off_b0;
     d.off_db = d.off_b0 + d.red_rows * 16 * d.ncfg;
     d.off_stage = d.off_b0 + work;                        // staging: [C * n * n] G, [C * n] u
-    d.tab_bytes = ((2 * 2 * (1 << (n - 1)) + 4 * 64 + 2 * d.zrec) + 15) & ~15;   // mask16, rank16, lvlT, lvlZ, recSQ
+    d.tab_bytes = ((2 * 2 * d.zrec + 4 * 32) + 15) & ~15;   // rank16, recSQ (ground set Q), lvlZ
     d.smem_bytes = (size_t)d.tab_bytes + sizeof(double) * (size_t)(d.off_stage + C * n * n + C * n);
     return d;
 }
@@ -254,7 +256,7 @@ __device__ __forceinline__ void pair_dispatch_item(const PairLevel& L, unsigned 
 #define COS_PAIR_CASE(K) case K - 1: if (K <= MAXNC) { pair_item<C, (K <= MAXNC ? K : 1)>(L, SQ, x, u, sm, Wl, lanes); break; }
     switch (N) {
         COS_PAIR_CASE(1) COS_PAIR_CASE(2) COS_PAIR_CASE(3) COS_PAIR_CASE(4) COS_PAIR_CASE(5)
-        COS_PAIR_CASE(6) COS_PAIR_CASE(7) COS_PAIR_CASE(8)
+        COS_PAIR_CASE(6) COS_PAIR_CASE(7) COS_PAIR_CASE(8) COS_PAIR_CASE(9)
         default: pair_item<C, MAXNC>(L, SQ, x, u, sm, Wl, lanes); break;
     }
 #undef COS_PAIR_CASE
@@ -349,11 +351,12 @@ __global__ void __launch_bounds__(MAXT, MINB) eval_pair_kernel(EvalArgs a, PairD
 #ifdef COS_PHASE_TIMING
     long long phase_t0__ = clock64();
 #endif
-    uint16_t* mask16 = reinterpret_cast<uint16_t*>(smem_raw);
-    uint16_t* rank16 = mask16 + (1 << (d.n - 1));
-    int* lvlT = reinterpret_cast<int*>(rank16 + (1 << (d.n - 1)));   // list offsets, ground set n-1 bits
-    int* lvlZ = lvlT + 32;                                           // Z record offsets, ground set qmax bits
-    uint16_t* recSQ = reinterpret_cast<uint16_t*>(lvlZ + 32);        // Z record -> S_Q
+    // subsets of Q by popcount in colex order (rank independent of the ground set): rank16[mask], recSQ[lvlZ[|S|] + rank]
+    uint16_t* rank16 = reinterpret_cast<uint16_t*>(smem_raw);
+    uint16_t* recSQ = rank16 + (1 << d.qmax);                        // Z record -> S_Q (also the reduction's row lists)
+    int* lvlZ = reinterpret_cast<int*>(recSQ + (1 << d.qmax));       // Z record offsets, ground set qmax bits
+    const uint16_t* mask16 = recSQ;
+    const int* lvlT = lvlZ;
     double* smd = reinterpret_cast<double*>(smem_raw + d.tab_bytes);
     const int tid = threadIdx.x, nthreads = blockDim.x;
     const int n = d.n, qmax = d.qmax, nsp = d.nsp;
@@ -365,21 +368,17 @@ __global__ void __launch_bounds__(MAXT, MINB) eval_pair_kernel(EvalArgs a, PairD
     double* sm = smd + (2 * g + u) * 2;
     const double* Wl = smd + d.off_w + rep * C + g;
 
-    // ---- tables: subsets of {0..n-2} by popcount in colex order (rank independent of the ground set) ----
     if (tid == 0) {
         int run = 0;
-        for (int j = 0; j <= n; ++j) { lvlT[j] = run; run += kBinom.c[n - 1][j]; }
-        run = 0;
         for (int j = 0; j <= qmax + 1; ++j) { lvlZ[j] = run; run += kBinom.c[qmax][j]; }
     }
     __syncthreads();
-    for (unsigned mk = tid; mk < (1u << (n - 1)); mk += nthreads) {
+    for (unsigned mk = tid; mk < (1u << qmax); mk += nthreads) {
         int rk = 0, i = 0;
         unsigned m = mk;
         while (m) { const int s = __ffs(m) - 1; m &= m - 1; ++i; rk += kBinom.c[s][i]; }
         rank16[mk] = (uint16_t)rk;
-        mask16[lvlT[i] + rk] = (uint16_t)mk;
-        if (mk < (1u << qmax)) recSQ[lvlZ[i] + rk] = (uint16_t)mk;
+        recSQ[lvlZ[i] + rk] = (uint16_t)mk;
     }
     __syncthreads();
 
@@ -451,7 +450,7 @@ __global__ void __launch_bounds__(MAXT, MINB) eval_pair_kernel(EvalArgs a, PairD
             team_reduce<C>(CB, DB, ncfg, n, mask16, lvlT, tid, nthreads);
             COS_PHASE_MARK(13);
             if (tid < ncfg) a.out[cfgbase + tid] = CB[red_elem<C>((NS >> (1 + kRedLB)) - 1, 15u, tid)];
-        } else {
+        } else if constexpr (C >= 2) {
             pair_combine<C, C / 2>(smd, d, ncfg, recSQ, tid, nthreads);
             __syncthreads();
             COS_PHASE_MARK(12);
