@@ -75,6 +75,11 @@ def get_workload(name: str, rank: int = 0):
 
 
 # ----------------------------------------------------------------------------------------------
+# dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel, per launch, from the committed ncu capture
+# (profiles/r1c_launches_default_bench.md, "DRAM traffic"); None for workloads that were not captured.
+NCU_TRAFFIC = {"cfg3_n10_b16384": 13210368 + 23552}
+
+
 class ClockSampler:
     """Samples SM clocks and throttle reasons DURING the timed region.
 
@@ -382,7 +387,7 @@ def run_ours(args):
                      "peak_source": "cos_probe_dfma: register-only FP64 FMA kernel measured in this run "
                                     "(MEASURED_PEAKS.json has no FP64 figure); nominal 148 SM x 64 FMA/clk x 1.965 GHz = 37.2",
                      "kernel_ms": kern_ms, "kernel_launches_timed": kern_launches,
-                     "smem_probe_gbs": smem_gbs, "traffic": None},
+                     "smem_probe_gbs": smem_gbs, "traffic": NCU_TRAFFIC.get(w.name)},
     }
     if not args.no_cpu_baseline and world == 1:
         line["cpu_baseline"] = cpu_baseline(w)

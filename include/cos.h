@@ -90,13 +90,15 @@ int cos_eval_all(cos_ctx* ctx, int n, long long batch, const double* d_Gup, cons
 int cos_eval_connected(cos_ctx* ctx, int n, long long batch, const double* d_Gup, const double* d_Gdn,
                        const double* d_u, double U, double* d_out);
 
-/* Fused path a1..a5: vertices in, connected value out; G lives only in library scratch.
+/* Whole path a1..a5 in one call: vertices in, connected value out.  G is assembled into a buffer the
+ * context owns (grown on demand, freed by cos_destroy) and read back once by the evaluation kernel, i.e. the
+ * call is cos_build_G + cos_eval_connected without a caller-visible G (two kernel launches on the ctx stream).
  * Both species use their registered tables; if they share one table a single propagation is done.
  * Arguments as in cos_build_G / cos_eval_connected. */
 int cos_eval_connected_xt(cos_ctx* ctx, int n, long long batch, const int* d_xy, const double* d_tau,
                           double g_diag, const double* d_u, double U, double* d_out);
 
-/* The same fused path with HOST buffers (pinned memory recommended): copies h_xy, h_tau (and h_u if
+/* The same whole-path call with HOST buffers (pinned memory recommended): copies h_xy, h_tau (and h_u if
  * not NULL) to the device, runs a1..a5, copies the batch results back into h_out and synchronises
  * the stream before returning.  Used for end-to-end timing (h2d = batch*(8n + 8n [+ 8n]) bytes,
  * d2h = 8*batch bytes). */
