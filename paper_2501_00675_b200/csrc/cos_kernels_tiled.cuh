@@ -83,7 +83,7 @@ inline TiledDims tiled_dims(int n, int G, int nsp)
     if (work < need) work = need;
     d.cfg_doubles = d.wstride + nsp * d.zrec * RS + work;
     d.cfg_doubles = (d.cfg_doubles + 1) & ~1;
-    d.tab_bytes = ((2 * 2 * (1 << (n - 1)) + 4 * 64) + 15) & ~15;   // mask16 + rank16 (2^(n-1) each) + lvlT[32] + lvlZ[32]
+    d.tab_bytes = (((2 * 2 * (1 << (n - 1)) + 4 * 64) + 15) & ~15) + 4096;   // mask16 + rank16 (2^(n-1) each) + lvlT[32] + lvlZ[32] + wtab[512]
     return d;
 }
 
@@ -513,16 +513,28 @@ __global__ void __launch_bounds__(THREADS) eval_tiled_kernel(EvalArgs a, TiledDi
         //      D1[U] = D[2U], both in the padded block layout of cos_reduce_blocked.cuh ----
         const int off_c = off_b0;
         const int off_d1 = off_b0 + red_rows(n) * kRowStride;
-        for (unsigned t = tid; t < (unsigned)ng * N; t += THREADS) {
-            const unsigned g = t >> n, S = t & (N - 1);
+        double* wtab = reinterpret_cast<double*>(smem_raw + d.tab_bytes - 4096);   // w(S) = wtab[S & 255] * wtab[256 + (S >> 8)]
+        for (int g = 0; g < ng; ++g) {
             double* cfg = cfg0 + (size_t)g * d.cfg_doubles;
-            const unsigned SQ = S >> B, ST = S & (NT - 1);
-            const int rec = lvl[__popc(SQ)] + rank16[SQ];
-            const double zu = cfg[off_z + (size_t)rec * RS + ST];
-            const double zd = cfg[off_z + (size_t)(nsp - 1) * d.zrec * RS + (size_t)rec * RS + ST];
-            double w = 1.0;
-            if (nsp == 1) { unsigned mm = S; while (mm) { const int v = __ffs(mm) - 1; mm &= mm - 1; w *= cfg[off_w + n * n + v]; } }
-            cfg[((S & 1u) ? off_c : off_d1) + red_addr(S >> 1)] = w * zu * zd;
+            if (nsp == 1) {
+                __syncthreads();
+                for (int t = tid; t < 512; t += THREADS) {
+                    const int vb = (t >> 8) * 8;
+                    unsigned mm = (unsigned)t & 255u;
+                    double w = 1.0;
+                    while (mm) { const int v = vb + __ffs(mm) - 1; mm &= mm - 1; if (v < n) w *= cfg[off_w + n * n + v]; }
+                    wtab[t] = w;
+                }
+                __syncthreads();
+            }
+            for (unsigned S = tid; S < N; S += THREADS) {
+                const unsigned SQ = S >> B, ST = S & (NT - 1);
+                const int rec = lvl[__popc(SQ)] + rank16[SQ];
+                const double zu = cfg[off_z + (size_t)rec * RS + ST];
+                const double zd = cfg[off_z + (size_t)(nsp - 1) * d.zrec * RS + (size_t)rec * RS + ST];
+                const double w = (nsp == 1) ? wtab[S & 255u] * wtab[256u + (S >> 8)] : 1.0;
+                cfg[((S & 1u) ? off_c : off_d1) + red_addr(S >> 1)] = w * zu * zd;
+            }
         }
         __syncthreads();
         COS_PHASE_MARK(2);

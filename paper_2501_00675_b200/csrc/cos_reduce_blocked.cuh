@@ -6,7 +6,7 @@
 // S' = (hi, lo) with lo = the 4 lowest bits.  A "leaf" multiplies the 16-value block C'[T_hi, .] with the
 // block D1[U_hi, .] as a subset convolution over lo: 81 FMAs on 32 loaded values, all in registers.
 //   out[S_hi, .] = sum over T_hi subset of S_hi (T_hi != S_hi) of leaf(C'[T_hi], D1[S_hi \ T_hi])
-// followed by a 65-FMA in-register solve of the diagonal block (T_hi = S_hi), level by level in |S_hi|.
+// level by level in |S_hi|; the diagonal block (T_hi = S_hi) is made the identity beforehand (see the code).
 // The 2^|S_hi| terms of one output are split over 2^s adjacent lanes (s chosen per level so that the CTA
 // is filled); the lane owns the sub-subsets of s chosen vertices of S_hi, partial blocks are summed by a
 // recursive-halving shuffle exchange.  Blocks are rows of 18 doubles (144 B) whose row index is XOR-folded
@@ -55,7 +55,45 @@ __device__ __forceinline__ void reduce_blocked_rt(double* cfg0, int cfg_doubles,
                                                   const uint16_t* mask16, const int* lvlT, int tid, const int THREADS)
 {
     const int hb = n - 1 - kLB;
-    for (int l = 0; l <= hb; ++l) {
+    // ---- identity diagonal block: with g = (D1[hi = {}])^-1 over lo, C' = (D0 * g) / (D1 * g) and
+    //      (D1 * g)[hi = {}] = delta, so no output row needs a triangular solve of its own ----
+    if (tid < ng) {
+        double* Dg = cfg0 + (size_t)tid * cfg_doubles + off_d1;
+        double e[16], gi[16];
+        load_block(Dg, e);                               // red_phys_row(0) == 0
+        gi[0] = 1.0;                                     // D[{}] = 1
+#pragma unroll
+        for (int lo = 1; lo < 16; ++lo) {
+            double v = 0.0;
+#pragma unroll
+            for (int T = 0; T < 16; ++T)
+                if ((T & ~lo) == 0 && T != lo) v = fma(-gi[T], e[lo ^ T], v);
+            gi[lo] = v;
+        }
+#pragma unroll
+        for (int t = 0; t < 16; t += 2) *reinterpret_cast<double2*>(Dg + t) = make_double2(gi[t], gi[t + 1]);
+    }
+    __syncthreads();
+    {
+        const int rows = 1 << hb;
+        const int per_cfg = 2 * rows - 1;
+        for (int task = tid; task < ng * per_cfg; task += THREADS) {
+            const int g = task / per_cfg, r = task - g * per_cfg;
+            double* base = cfg0 + (size_t)g * cfg_doubles;
+            double* row = (r < rows) ? base + off_c + red_phys_row((unsigned)r) * kRowStride
+                                     : base + off_d1 + red_phys_row((unsigned)(r - rows + 1)) * kRowStride;
+            double gi[16], v[16], o[16];
+            load_block(base + off_d1, gi);
+            load_block(row, v);
+#pragma unroll
+            for (int t = 0; t < 16; ++t) o[t] = 0.0;
+            leaf_conv(v, gi, o);
+#pragma unroll
+            for (int t = 0; t < 16; t += 2) *reinterpret_cast<double2*>(row + t) = make_double2(o[t], o[t + 1]);
+        }
+    }
+    __syncthreads();
+    for (int l = 1; l <= hb; ++l) {
         const int cntl = kBinom.c[hb][l];
         const int outputs = ng * cntl;
         int s = l < 5 ? l : 5;
@@ -118,7 +156,10 @@ __device__ __forceinline__ void reduce_blocked_rt(double* cfg0, int cfg_doubles,
             if (s == 0) {
                 if (active) {
 #pragma unroll
-                    for (int t = 0; t < 16; ++t) acc[t] = blk[t] - acc[t];
+                    for (int t = 0; t < 16; t += 2) {
+                        const double2 d0 = *reinterpret_cast<const double2*>(blk + t);
+                        *reinterpret_cast<double2*>(blk + t) = make_double2(d0.x - acc[t], d0.y - acc[t + 1]);
+                    }
                 }
             } else {
                 double r8[8];
@@ -172,26 +213,6 @@ __device__ __forceinline__ void reduce_blocked_rt(double* cfg0, int cfg_doubles,
                         }
                     }
                 }
-                __syncwarp();
-                if (active && c == 0) {
-#pragma unroll
-                    for (int t = 0; t < 16; ++t) acc[t] = blk[t];
-                }
-            }
-            // ---- diagonal block: x[lo] = pre[lo] - sum_{T proper subset of lo} x[T] e[lo ^ T], e = D1[hi = {}] ----
-            if (active && c == 0) {
-                double e[16];
-                load_block(Dg, e);                       // red_phys_row(0) == 0
-#pragma unroll
-                for (int lo = 1; lo < 16; ++lo) {
-                    double v = acc[lo];
-#pragma unroll
-                    for (int T = 0; T < 16; ++T)
-                        if ((T & ~lo) == 0 && T != lo) v = fma(-acc[T], e[lo ^ T], v);
-                    acc[lo] = v;
-                }
-#pragma unroll
-                for (int t = 0; t < 16; t += 2) *reinterpret_cast<double2*>(blk + t) = make_double2(acc[t], acc[t + 1]);
             }
         }
         __syncthreads();
