@@ -115,7 +115,7 @@ inline TeamDims team_dims(int n, int nsp)
     d.red_rows = 1 << (n - 1 - kRedLB);
     d.off_w = 0;
     d.off_u = d.off_w + n * n * L::WE;
-    d.off_z = d.off_u + 16 * d.ncfg;                      // un[v][cfg] = -u_v
+    d.off_z = d.off_u + 40 * d.ncfg;                      // un[v][cfg] = -u_v, then the 16 + 8 products of team_combine
     d.off_b0 = d.off_z + d.zrec * L::REC;
     int work = 2 * maxrec * L::REC;
     const int need = 2 * d.red_rows * 16 * d.ncfg;
@@ -572,7 +572,6 @@ __device__ __forceinline__ void team_combine(double* smd, const TeamDims& d, int
     double* DB = smd + d.off_db;
     const double* un = smd + d.off_u;
     const int cg = tid % NC;
-    if (cg >= ncfg) return;
     double wT[8];
 #pragma unroll
     for (int t = 0; t < 8; ++t) wT[t] = 1.0;
@@ -581,13 +580,20 @@ __device__ __forceinline__ void team_combine(double* smd, const TeamDims& d, int
 #pragma unroll
         for (int t = 0; t < 8; ++t) wT[t] = ((t & 1) ? u0 : 1.0) * ((t & 2) ? u1 : 1.0) * ((t & 4) ? u2 : 1.0);
     }
+    // w(S_Q) = wt[S_Q & 15] * wt[16 + (S_Q >> 4)]: products over the 4 low / 3 high vertices of Q, built once per team
+    double* wt = smd + d.off_u + 16 * NC;
+    if (NSP == 1) {
+        for (int t = tid / NC; t < 24; t += nthreads / NC) {
+            unsigned m = t < 16 ? (unsigned)t : (unsigned)(t - 16) << 4;
+            double w = 1.0;
+            while (m) { const int v = __ffs(m) - 1; m &= m - 1; if (v < d.qmax) w *= un[(v + kTeamB) * NC + cg]; }
+            wt[t * NC + cg] = w;
+        }
+        team_sync(nthreads);
+    }
     for (int rec = tid / NC; rec < d.zrec; rec += nthreads / NC) {
         const unsigned SQ = recSQ[rec];
-        double wq = 1.0;
-        if (NSP == 1) {
-            unsigned m = SQ;
-            while (m) { const int v = __ffs(m) - 1; m &= m - 1; wq *= un[(v + kTeamB) * NC + cg]; }
-        }
+        const double wq = (NSP == 1) ? wt[(SQ & 15u) * NC + cg] * wt[(16u + (SQ >> 4)) * NC + cg] : 1.0;
         const RecPtr<C> zp(smd + d.off_z + (cg * NSP) * 2, rec);
         double val[8];
 #pragma unroll
