@@ -125,7 +125,7 @@ inline TeamDims team_dims(int n, int nsp)
     d.off_db = d.off_b0 + d.red_rows * 16 * d.ncfg;
     d.off_stage = d.off_b0 + work;                        // staging: [C * n * n] G, [C * n] u
     d.dsc_off = ((2 * 2 * (1 << (n - 1)) + 4 * 64 + 2 * d.zrec) + 31) & ~31;     // mask16, rank16, lvlT, lvlZ, recSQ
-    d.tab_bytes = d.dsc_off + 32 * d.zrec;                                        // + one 32-byte descriptor per pattern
+    d.tab_bytes = d.dsc_off + 32 * d.zrec + 512;                                  // + one 32-byte descriptor per pattern + column units of levels 0, 1
     d.smem_bytes = (size_t)d.tab_bytes + sizeof(double) * (size_t)(d.off_stage + C * n * n + C * n);
     return d;
 }
@@ -300,6 +300,93 @@ __device__ __forceinline__ void team_item(const TeamLevel& L, const uint32_t* ds
         for (int p = 0; p < 4; ++p)
             *reinterpret_cast<double2*>(o.part(p)) = make_double2(-acc[2 * p][N], -acc[2 * p + 1][N]);
     }
+}
+
+// Column item: ONE column k (Q-target k < Nown, or the close k == Nown) of pattern S_Q.  Used for the first levels,
+// where a pattern has few sources but many targets: the whole-pattern item is then a long serial instruction
+// stream on a handful of lanes while the other warps wait at the level barrier.  Every column thread repeats the
+// T-target part (12 of its 20 FMAs per source), which costs FP64 issue slots nobody else wants at these levels
+// and cuts the critical path of the level by the number of columns.
+template <int C>
+__device__ __forceinline__ void team_item_col(const TeamLevel& L, const uint32_t* dsc, int x, int k, double* sm,
+                                              const double* Wl)
+{
+    using Lay = TeamLayout<C>;
+    constexpr int WE = Lay::WE, NT = kTeamNT, B = kTeamB;
+    const int n = L.n;
+    const uint32_t w0 = dsc[0], w4 = dsc[4];
+    unsigned srcs = dsc[5];
+    const int zrec = (int)(w0 >> 16);
+    const int h = (int)((w4 >> 24) & 15u);
+    const int nown = (int)(w4 >> 28);
+    const bool close = (k == nown);
+    const int colo = (close ? h : (int)((w4 >> (4 * k)) & 15u)) * WE;
+    const int rowstride = n * WE;
+    double acc[NT], accT[NT][B];
+    {
+        const RecPtr<C> zp(sm + L.off_z, zrec);
+        double a[NT];
+        team_load_rec<C>(zp, a);
+        const double* row = Wl + h * rowstride;
+        const double w = row[colo];
+#pragma unroll
+        for (int t = 0; t < NT; ++t) acc[t] = a[t] * w;
+#pragma unroll
+        for (int tp = 0; tp < B; ++tp) {
+            const double wt = row[tp * WE];
+#pragma unroll
+            for (int t = 0; t < NT; ++t) accT[t][tp] = ((t >> tp) & 1) ? 0.0 : a[t] * wt;
+        }
+    }
+    {
+        int rec = x;
+        for (int i = 0; i < L.j; ++i) {
+            const int v = (int)(srcs & 15u);
+            srcs >>= 4;
+            const RecPtr<C> rp(sm + L.off_cur, rec);
+            rec += L.cnt;
+            const double* row = Wl + v * rowstride;
+            double a[NT];
+            team_load_rec<C>(rp, a);
+            const double w = row[colo];
+#pragma unroll
+            for (int t = 0; t < NT; ++t) acc[t] = fma(a[t], w, acc[t]);
+#pragma unroll
+            for (int tp = 0; tp < B; ++tp) {
+                const double wt = row[tp * WE];
+#pragma unroll
+                for (int t = 0; t < NT; ++t)
+                    if (!((t >> tp) & 1)) accT[t][tp] = fma(a[t], wt, accT[t][tp]);
+            }
+        }
+    }
+#pragma unroll
+    for (int l = 1; l < B; ++l)
+#pragma unroll
+        for (int t = 0; t < NT; ++t) {
+            if (cpopc(t) != l) continue;
+#pragma unroll
+            for (int ts = 0; ts < B; ++ts) {
+                if (!((t >> ts) & 1)) continue;
+                const double sv = accT[t ^ (1 << ts)][ts];
+#pragma unroll
+                for (int tp = 0; tp < B; ++tp)
+                    if (!((t >> tp) & 1)) accT[t][tp] = fma(sv, Wl[(ts * n + tp) * WE], accT[t][tp]);
+            }
+        }
+#pragma unroll
+    for (int ts = 0; ts < B; ++ts) {
+        const double w = Wl[ts * rowstride + colo];
+#pragma unroll
+        for (int t = 0; t < NT; ++t)
+            if ((t >> ts) & 1) acc[t] = fma(accT[t ^ (1 << ts)][ts], w, acc[t]);
+    }
+    const double sg = close ? -1.0 : 1.0;             // Z = -close (one -1 per closed fermion loop)
+    const int orec = close ? L.lvlZ_j1 + x : (int)reinterpret_cast<const uint16_t*>(dsc + 1)[k];
+    const RecPtr<C> o(sm + (close ? L.off_z : L.off_nxt), orec);
+#pragma unroll
+    for (int p = 0; p < 4; ++p)
+        *reinterpret_cast<double2*>(o.part(p)) = make_double2(sg * acc[2 * p], sg * acc[2 * p + 1]);
 }
 
 template <int C>
@@ -719,12 +806,26 @@ __global__ void __launch_bounds__(MAXT, MINB) eval_team_kernel(EvalArgs a, TeamD
     __syncthreads();
     uint32_t* dtab = reinterpret_cast<uint32_t*>(smem_raw + d.dsc_off);
     for (int r = 1 + tid; r < (1 << qmax); r += nthreads) team_build_descriptor(dtab + r * 8, recSQ[r], qmax, lvlZ, rank16);
+    // column units (pattern x | column << 8) of level 0, their count in ucol[254]
+    uint16_t* ucol = reinterpret_cast<uint16_t*>(smem_raw + d.dsc_off + 32 * d.zrec);
+    __syncthreads();
+    if (tid == 0) {
+        int u = 0;
+        for (int j = 0; j < 1; ++j) {
+            for (int x = 0; x < kBinom.c[qmax][j + 1]; ++x) {
+                const int nown = (int)(dtab[(lvlZ[j + 1] + x) * 8 + 4] >> 28);
+                for (int k = 0; k <= nown && u < 254; ++k) ucol[u++] = (uint16_t)(x | (k << 8));
+            }
+            ucol[254 + j] = (uint16_t)u;
+        }
+    }
 
     double* stage = smd + d.off_stage;
     if ((long long)blockIdx.x < nteams) {
         const long long nx0 = (long long)blockIdx.x * C;
         team_prefetch_inputs<C>(a, n, nsp, stage, nx0, (int)min((long long)C, total_inst - nx0), tid, nthreads);
     }
+    const bool col_ok = qmax >= 2 && qmax <= 7;      // unit table: 28 + 91 entries at most (order 10)
     for (long long team = blockIdx.x; team < nteams; team += gridDim.x) {
         const long long inst0 = team * C;
         const int ninst = (int)min((long long)C, total_inst - inst0);
@@ -754,6 +855,16 @@ __global__ void __launch_bounds__(MAXT, MINB) eval_team_kernel(EvalArgs a, TeamD
             L.cnt_next = kBinom.c[qmax][j + 2];
             L.lvlZ_j = lvlZ[j]; L.lvlZ_j1 = lvlZ[j + 1];
             L.off_cur = cur; L.off_nxt = nxt;
+            if (j == 0 && col_ok) {      // measured: column items win at level 0 only (level 1 needs three passes)
+                const int ub = 0, ue = (int)ucol[254];
+                for (int u0 = ub; u0 < ue; u0 += d.pslots) {
+                    const int u = u0 + slot;
+                    if (u < ue && g < ninst) {
+                        const int xk = (int)ucol[u];
+                        team_item_col<C>(L, dtab + (L.lvlZ_j1 + (xk & 255)) * 8, xk & 255, xk >> 8, sm, Wl);
+                    }
+                }
+            } else
             for (int x0 = 0; x0 < L.cnt; x0 += d.pslots) {
                 const int x = x0 + slot;
                 const bool active = (x < L.cnt) && (g < ninst);
