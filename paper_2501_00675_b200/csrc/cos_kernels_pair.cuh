@@ -368,6 +368,14 @@ __global__ void __launch_bounds__(MAXT, MINB) eval_pair_kernel(EvalArgs a, PairD
     double* sm = smd + (2 * g + u) * 2;
     const double* Wl = smd + d.off_w + rep * C + g;
 
+    // the first team's inputs are fetched while the tables are being built
+    double* stage = smd + d.off_stage;
+    {
+        const long long total_inst0 = a.batch * nsp;
+        const long long nx0 = (long long)blockIdx.x * C;
+        if (nx0 < total_inst0)
+            team_prefetch_inputs<C>(a, n, nsp, stage, nx0, (int)min((long long)C, total_inst0 - nx0), tid, nthreads);
+    }
     if (tid == 0) {
         int run = 0;
         for (int j = 0; j <= qmax + 1; ++j) { lvlZ[j] = run; run += kBinom.c[qmax][j]; }
@@ -384,11 +392,6 @@ __global__ void __launch_bounds__(MAXT, MINB) eval_pair_kernel(EvalArgs a, PairD
 
     const long long total_inst = a.batch * nsp;
     const long long nteams = (total_inst + C - 1) / C;
-    double* stage = smd + d.off_stage;
-    if ((long long)blockIdx.x < nteams) {
-        const long long nx0 = (long long)blockIdx.x * C;
-        team_prefetch_inputs<C>(a, n, nsp, stage, nx0, (int)min((long long)C, total_inst - nx0), tid, nthreads);
-    }
     for (long long team = blockIdx.x; team < nteams; team += gridDim.x) {
         const long long inst0 = team * C;
         const int ninst = (int)min((long long)C, total_inst - inst0);

@@ -787,6 +787,12 @@ __global__ void __launch_bounds__(MAXT, MINB) eval_team_kernel(EvalArgs a, TeamD
     double* sm = smd + g * 2;
     const double* Wl = smd + d.off_w + rep * C + g;
 
+    // the first team's inputs are fetched while the tables below are being built
+    double* stage = smd + d.off_stage;
+    if ((long long)blockIdx.x < nteams) {
+        const long long nx0 = (long long)blockIdx.x * C;
+        team_prefetch_inputs<C>(a, n, nsp, stage, nx0, (int)min((long long)C, total_inst - nx0), tid, nthreads);
+    }
     // ---- tables: subsets of {0..n-2} by popcount in colex order (rank independent of the ground set) ----
     if (tid == 0) {
         int run = 0;
@@ -820,11 +826,6 @@ __global__ void __launch_bounds__(MAXT, MINB) eval_team_kernel(EvalArgs a, TeamD
         }
     }
 
-    double* stage = smd + d.off_stage;
-    if ((long long)blockIdx.x < nteams) {
-        const long long nx0 = (long long)blockIdx.x * C;
-        team_prefetch_inputs<C>(a, n, nsp, stage, nx0, (int)min((long long)C, total_inst - nx0), tid, nthreads);
-    }
     const bool col_ok = qmax >= 2 && qmax <= 7;      // unit table: 28 + 91 entries at most (order 10)
     for (long long team = blockIdx.x; team < nteams; team += gridDim.x) {
         const long long inst0 = team * C;
