@@ -568,11 +568,31 @@ __device__ __forceinline__ void team_reduce(double* CB, double* DB, int ncfg, in
                         double cb[16], db[16];
                         red_load_block<NC>(CB, T, cg, cb);
                         red_load_block<NC>(DB, S ^ T, cg, db);
-                        leaf_conv(cb, db, acc);
+                        if (l == hb) {
+                            // top row: only C'[full] = element lo = 15 is ever read (a5), 16 of the 81 products
+                            double p0 = 0.0, p1 = 0.0, p2 = 0.0, p3 = 0.0;
+#pragma unroll
+                            for (int t = 0; t < 16; t += 4) {
+                                p0 = fma(cb[t], db[15 ^ t], p0);
+                                p1 = fma(cb[t + 1], db[15 ^ (t + 1)], p1);
+                                p2 = fma(cb[t + 2], db[15 ^ (t + 2)], p2);
+                                p3 = fma(cb[t + 3], db[15 ^ (t + 3)], p3);
+                            }
+                            acc[15] += (p0 + p1) + (p2 + p3);
+                        } else {
+                            leaf_conv(cb, db, acc);
+                        }
                     }
                     if (Th == 0) break;
                     Th = (Th - 1) & rest;
                 }
+            }
+            if (l == hb) {
+                // one value per lane: plain butterfly sum over the 2^s lanes of the output, then C'[full] -= sum
+                double v = acc[15];
+                for (int k = 0; k < s; ++k) v += __shfl_xor_sync(0xffffffffu, v, (NC << k) & 31);
+                if (active && c == 0) { const int e = red_elem<NC>(S, 15u, cg); CB[e] = CB[e] - v; }
+                continue;
             }
             // ---- sum the 2^s partial blocks: recursive halving, lane bit k keeps lo-bit k == its own bit ----
             double* blk = CB;     // element lo at blk[red_elem(S, lo, cg)]
