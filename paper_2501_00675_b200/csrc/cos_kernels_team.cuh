@@ -77,7 +77,7 @@ struct TeamDims {
     int red_rows;      // 2^(n-1-kRedLB) block rows of the reduction arrays
     int off_w, off_u, off_z, off_b0, off_b1;   // double offsets behind the tables
     int off_cb, off_db;                        // reduction arrays (alias the frontier buffers)
-    int off_stage;                             // staging buffer: G and u of the next team (cp.async)
+    int off_stage;                             // staging buffer: u of the next team (cp.async)
     int dsc_off;                               // byte offset of the item descriptors inside the table area
     int tab_bytes;
     size_t smem_bytes;
@@ -123,10 +123,10 @@ inline TeamDims team_dims(int n, int nsp)
     d.off_b1 = d.off_b0 + maxrec * L::REC;
     d.off_cb = d.off_b0;
     d.off_db = d.off_b0 + d.red_rows * 16 * d.ncfg;
-    d.off_stage = d.off_b0 + work;                        // staging: [C * n * n] G, [C * n] u
+    d.off_stage = d.off_b0 + work;                        // staging: [C * n] u of the next team
     d.dsc_off = ((2 * 2 * (1 << (n - 1)) + 4 * 64 + 2 * d.zrec) + 31) & ~31;     // mask16, rank16, lvlT, lvlZ, recSQ
     d.tab_bytes = d.dsc_off + 32 * d.zrec + 512;                                  // + one 32-byte descriptor per pattern + column units of levels 0, 1
-    d.smem_bytes = (size_t)d.tab_bytes + sizeof(double) * (size_t)(d.off_stage + C * n * n + C * n);
+    d.smem_bytes = (size_t)d.tab_bytes + sizeof(double) * (size_t)(d.off_stage + C * n);
     return d;
 }
 
@@ -682,14 +682,14 @@ __device__ __forceinline__ void team_combine(double* smd, const TeamDims& d, int
     double wT[8];
 #pragma unroll
     for (int t = 0; t < 8; ++t) wT[t] = 1.0;
-    if (NSP == 1) {
+    {
         const double u0 = un[0 * NC + cg], u1 = un[1 * NC + cg], u2 = un[2 * NC + cg];
 #pragma unroll
         for (int t = 0; t < 8; ++t) wT[t] = ((t & 1) ? u0 : 1.0) * ((t & 2) ? u1 : 1.0) * ((t & 4) ? u2 : 1.0);
     }
     // w(S_Q) = wt[S_Q & 15] * wt[16 + (S_Q >> 4)]: products over the 4 low / 3 high vertices of Q, built once per team
     double* wt = smd + d.off_u + 16 * NC;
-    if (NSP == 1) {
+    {
         for (int t = tid / NC; t < 24; t += nthreads / NC) {
             unsigned m = t < 16 ? (unsigned)t : (unsigned)(t - 16) << 4;
             double w = 1.0;
@@ -700,7 +700,7 @@ __device__ __forceinline__ void team_combine(double* smd, const TeamDims& d, int
     }
     for (int rec = tid / NC; rec < d.zrec; rec += nthreads / NC) {
         const unsigned SQ = recSQ[rec];
-        const double wq = (NSP == 1) ? wt[(SQ & 15u) * NC + cg] * wt[(16u + (SQ >> 4)) * NC + cg] : 1.0;
+        const double wq = wt[(SQ & 15u) * NC + cg] * wt[(16u + (SQ >> 4)) * NC + cg];
         const RecPtr<C> zp(smd + d.off_z + (cg * NSP) * 2, rec);
         double val[8];
 #pragma unroll
@@ -780,6 +780,51 @@ __device__ __forceinline__ void team_unpack_inputs(const EvalArgs& a, int n, int
         }
 }
 
+// Team kernel: the next team's matrices go straight into the replicated W with cp.async, issued as soon as the
+// last propagation level has released W (the combine and the reduction do not read it), so that a team starts with
+// its W in place -- no staging pass.  Only the couplings (a few values) are staged.
+template <int C, int REP>
+__device__ __forceinline__ void team_prefetch_w(const EvalArgs& a, int n, int nsp, double* Wd, double* stage_u,
+                                                long long inst0, int ninst, int tid, int nthreads)
+{
+    // nthreads is a multiple of C: a thread always serves the same instance gi, and the entries e0, e0 + step, ..
+    constexpr int WE = REP * C;
+    const int nn = n * n;
+    const int gi = tid % C, e0 = tid / C, step = nthreads / C;
+    double* w = Wd + gi;
+    if (gi < ninst) {
+        const long long b = (inst0 + gi) >> (nsp - 1);                // nsp is 1 or 2
+        const double* src = (((inst0 + gi) & (nsp - 1)) == 0 ? a.Gup : a.Gdn) + b * nn;
+        for (int e = e0; e < nn; e += step) {
+#pragma unroll
+            for (int r = 0; r < REP; ++r) cp_async8(w + e * WE + r * C, src + e);
+        }
+    } else {
+        for (int e = e0; e < nn; e += step) {
+#pragma unroll
+            for (int r = 0; r < REP; ++r) w[e * WE + r * C] = 0.0;
+        }
+    }
+    if (a.u) {
+        const long long cfg0 = inst0 >> (nsp - 1);
+        const int ncfg = ninst >> (nsp - 1);
+        for (int t = tid; t < ncfg * n; t += nthreads) cp_async8(stage_u + t, a.u + cfg0 * n + t);
+    }
+    cp_async_commit();
+}
+
+// un[v * NCt + cg] = -u_v of configuration cg of the team (0 for empty slots)
+template <int C>
+__device__ __forceinline__ void team_set_couplings(const EvalArgs& a, int n, int nsp, const double* stage_u, double* un,
+                                                   int ninst, int tid, int nthreads)
+{
+    const int NCt = C / nsp, ncfg = ninst / nsp;
+    for (int t = tid; t < NCt * n; t += nthreads) {
+        const int cg = t % NCt, v = t / NCt;
+        un[t] = (cg < ncfg) ? -(a.u ? stage_u[cg * n + v] : a.U) : 0.0;
+    }
+}
+
 template <int C, int MAXT, int MINB>
 __global__ void __launch_bounds__(MAXT, MINB) eval_team_kernel(EvalArgs a, TeamDims d)
 {
@@ -811,7 +856,7 @@ __global__ void __launch_bounds__(MAXT, MINB) eval_team_kernel(EvalArgs a, TeamD
     double* stage = smd + d.off_stage;
     if ((long long)blockIdx.x < nteams) {
         const long long nx0 = (long long)blockIdx.x * C;
-        team_prefetch_inputs<C>(a, n, nsp, stage, nx0, (int)min((long long)C, total_inst - nx0), tid, nthreads);
+        team_prefetch_w<C, REP>(a, n, nsp, smd + d.off_w, stage, nx0, (int)min((long long)C, total_inst - nx0), tid, nthreads);
     }
     // ---- tables: subsets of {0..n-2} by popcount in colex order (rank independent of the ground set) ----
     if (tid == 0) {
@@ -854,13 +899,8 @@ __global__ void __launch_bounds__(MAXT, MINB) eval_team_kernel(EvalArgs a, TeamD
         const int NCt = C / nsp;                 // configuration slots of a team
         const long long cfgbase = inst0 / nsp;
         cp_async_wait_all();
-        __syncthreads();
-        team_unpack_inputs<C, REP>(a, n, nsp, stage, smd + d.off_w, smd + d.off_u, ninst, tid, nthreads);
-        __syncthreads();
-        if (team + gridDim.x < nteams) {
-            const long long nx0 = (team + gridDim.x) * C;
-            team_prefetch_inputs<C>(a, n, nsp, stage, nx0, (int)min((long long)C, total_inst - nx0), tid, nthreads);
-        }
+        __syncthreads();          // W of this team is in place; the previous team's last reads are done
+        team_set_couplings<C>(a, n, nsp, stage, smd + d.off_u, ninst, tid, nthreads);
         COS_PHASE_MARK_T(0, nthreads);
         if (tid < ninst) team_small_stages<C>(smd + d.off_w + tid, n, smd + d.off_z + tid * 2);
         team_sync(nthreads);
@@ -896,6 +936,12 @@ __global__ void __launch_bounds__(MAXT, MINB) eval_team_kernel(EvalArgs a, TeamD
             const int tmp = cur; cur = nxt; nxt = tmp;
         }
 
+        // W is dead from here on: fetch the next team's matrices into it (the barrier of the last level is behind us;
+        // the couplings of THIS team were copied out of the staging area before the levels)
+        if (team + gridDim.x < nteams) {
+            const long long nx0 = (team + gridDim.x) * C;
+            team_prefetch_w<C, REP>(a, n, nsp, smd + d.off_w, stage, nx0, (int)min((long long)C, total_inst - nx0), tid, nthreads);
+        }
         // ---- a3 + a5 ("all"): D[full] = w * Zup[full] * Zdn[full] ----
         if (!a.connected) {
             if (tid < ncfg) {
@@ -905,7 +951,7 @@ __global__ void __launch_bounds__(MAXT, MINB) eval_team_kernel(EvalArgs a, TeamD
                 const double zu = zp[(tid * nsp) * 2];
                 const double zd = zp[(tid * nsp + nsp - 1) * 2];
                 double w = 1.0;
-                if (nsp == 1) for (int v = 0; v < n; ++v) w *= smd[d.off_u + v * NCt + tid];
+                for (int v = 0; v < n; ++v) w *= smd[d.off_u + v * NCt + tid];
                 a.out[cfgbase + tid] = w * zu * zd;
             }
             continue;
