@@ -795,10 +795,7 @@ __device__ __forceinline__ void team_prefetch_w(const EvalArgs& a, int n, int ns
     if (gi < ninst) {
         const long long b = (inst0 + gi) >> (nsp - 1);                // nsp is 1 or 2
         const double* src = (((inst0 + gi) & (nsp - 1)) == 0 ? a.Gup : a.Gdn) + b * nn;
-        for (int e = e0; e < nn; e += step) {
-#pragma unroll
-            for (int r = 0; r < REP; ++r) cp_async8(w + e * WE + r * C, src + e);
-        }
+        for (int e = e0; e < nn; e += step) cp_async8(w + e * WE, src + e);      // replica 0; team_replicate_w copies it
     } else {
         for (int e = e0; e < nn; e += step) {
 #pragma unroll
@@ -811,6 +808,23 @@ __device__ __forceinline__ void team_prefetch_w(const EvalArgs& a, int n, int ns
         for (int t = tid; t < ncfg * n; t += nthreads) cp_async8(stage_u + t, a.u + cfg0 * n + t);
     }
     cp_async_commit();
+}
+
+// Replicas 1..REP-1 of W from replica 0 (each thread copies the entries it fetched itself: no barrier in between).
+template <int C, int REP>
+__device__ __forceinline__ void team_replicate_w(int n, double* Wd, int ninst, int tid, int nthreads)
+{
+    constexpr int WE = REP * C;
+    if (REP == 1) return;
+    const int nn = n * n;
+    const int gi = tid % C, e0 = tid / C, step = nthreads / C;
+    if (gi >= ninst) return;
+    double* w = Wd + gi;
+    for (int e = e0; e < nn; e += step) {
+        const double v = w[e * WE];
+#pragma unroll
+        for (int r = 1; r < REP; ++r) w[e * WE + r * C] = v;
+    }
 }
 
 // un[v * NCt + cg] = -u_v of configuration cg of the team (0 for empty slots)
@@ -899,6 +913,7 @@ __global__ void __launch_bounds__(MAXT, MINB) eval_team_kernel(EvalArgs a, TeamD
         const int NCt = C / nsp;                 // configuration slots of a team
         const long long cfgbase = inst0 / nsp;
         cp_async_wait_all();
+        team_replicate_w<C, REP>(n, smd + d.off_w, ninst, tid, nthreads);
         __syncthreads();          // W of this team is in place; the previous team's last reads are done
         team_set_couplings<C>(a, n, nsp, stage, smd + d.off_u, ninst, tid, nthreads);
         COS_PHASE_MARK_T(0, nthreads);
