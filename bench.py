@@ -77,7 +77,7 @@ def get_workload(name: str, rank: int = 0):
 # ----------------------------------------------------------------------------------------------
 # dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel, per launch, from the committed ncu capture
 # (profiles/r1c_launches_default_bench.md, "DRAM traffic"); None for workloads that were not captured.
-NCU_TRAFFIC = {"cfg3_n10_b16384": 13210368 + 23552}
+NCU_TRAFFIC = {"cfg3_n10_b16384": 13198848 + 0}
 
 
 class ClockSampler:
