@@ -51,10 +51,17 @@ inline TiledDims big_dims(int n, int nsp)
     return d;
 }
 
+inline size_t pair_global_rec_doubles(int n);   // defined with the pair-kernel choices below
+
 // Doubles of global scratch per CTA (0: everything lives in shared memory).
 inline size_t eval_scratch_doubles(int n, int smem_optin)
 {
-    if (uses_big(n)) return (size_t)big_dims(n, 2).cfg_doubles;
+    if (uses_big(n)) {
+        size_t v = (size_t)big_dims(n, 2).cfg_doubles;
+        const size_t p = pair_global_rec_doubles(n);     // the pair kernel on global records (orders 14..16)
+        if (p > v) v = p;
+        return v;
+    }
     if (uses_tiled(n, 2, smem_optin)) return 0;
     if (!generic_needs_global(n, smem_optin)) return 0;
     return ((size_t)2 << n) + generic_frontier_doubles(n);
@@ -99,6 +106,18 @@ inline PairChoice pair_choice(int n, int nsp)
 // team sat on the critical path), and G costs 16 n^2 bytes per configuration of HBM traffic -- noise.
 inline bool has_fused_kernel(int, int, int) { return false; }
 
+// ---- pair kernel on global records (orders 14..16, one species): Z / frontier / reduction arrays in L2 scratch ----
+constexpr int kPairGlobalMinN = 14, kPairGlobalThreads = 256;
+inline bool uses_pair_global(int n, int nsp) { return n >= kPairGlobalMinN && n <= kMaxN && nsp == 1; }
+inline PairChoice pair_global_choice(int n)
+{
+    return {eval_pair_kernel<1, kPairGlobalThreads, 2, 8, true>, pair_dims_global<1>(n, kPairGlobalThreads)};
+}
+inline size_t pair_global_rec_doubles(int n)
+{
+    return (n >= kPairGlobalMinN && n <= kMaxN) ? (size_t)pair_global_choice(n).d.rec_doubles : 0;
+}
+
 using TiledKernel = void (*)(EvalArgs, TiledDims);
 inline TiledKernel tiled_kernel() { return eval_tiled_kernel<kTiledB, kTiledThreads, kTiledNA, kTiledJB, false>; }
 inline TiledKernel big_kernel() { return eval_tiled_kernel<kTiledB, kBigThreads, kBigNA, kBigJB, true>; }
@@ -116,6 +135,8 @@ inline cudaError_t configure_kernels(int smem_optin)
         e = cudaFuncSetAttribute(pair_choice(n, 1).fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
         if (e != cudaSuccess) return e;
     }
+    e = cudaFuncSetAttribute(pair_global_choice(kPairGlobalMinN).fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
+    if (e != cudaSuccess) return e;
     e = cudaFuncSetAttribute(big_kernel(), cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
     if (e != cudaSuccess) return e;
     return cudaFuncSetAttribute(tiled_kernel(), cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
@@ -158,6 +179,22 @@ inline cudaError_t dispatch_eval(const EvalArgs& a, cudaStream_t stream, int num
         }
     }
     if (a.fused) return cudaErrorInvalidValue;   // only the team and pair kernels assemble G on the fly
+    if (uses_pair_global(a.n, nsp) && a.scratch != nullptr) {
+        const PairChoice tc = pair_global_choice(a.n);
+        if (tc.d.smem_bytes <= (size_t)smem_optin && (size_t)tc.d.rec_doubles <= a.scratch_stride) {
+            int per_sm = 1;
+            cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, tc.fn, tc.d.threads, tc.d.smem_bytes);
+            if (e != cudaSuccess) return e;
+            if (per_sm < 1) per_sm = 1;
+            long long grid = (long long)num_sms * per_sm;
+            const long long cap = eval_max_ctas(a.n, a.batch, num_sms, smem_optin);
+            if (grid > cap) grid = cap;
+            if (grid > a.batch) grid = a.batch;
+            tc.fn<<<(unsigned)grid, tc.d.threads, tc.d.smem_bytes, stream>>>(a, tc.d);
+            *name = "eval_pair_kernel(global)";
+            return cudaGetLastError();
+        }
+    }
     if (uses_big(a.n)) {
         const TiledDims d = big_dims(a.n, nsp);
         const size_t smem = (size_t)d.tab_bytes;

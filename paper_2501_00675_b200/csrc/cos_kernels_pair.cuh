@@ -65,6 +65,7 @@ struct PairDims {
     int off_w, off_u, off_z, off_b0, off_b1;   // double offsets behind the tables
     int off_cb, off_db;                        // reduction arrays (alias the frontier buffers)
     int off_stage;                             // staging buffer: G and u of the next team (cp.async)
+    int rec_doubles;                           // doubles of the record space (W gap, -u, Z, frontier / reduction)
     int tab_bytes;
     size_t smem_bytes;
 };
@@ -101,7 +102,22 @@ inline PairDims pair_dims(int n, int nsp)
     d.off_cb = d.off_b0;
     d.off_db = d.off_b0 + d.red_rows * 16 * d.ncfg;
     d.off_stage = d.off_b0 + work;                        // staging: [C * n * n] G, [C * n] u
+    d.rec_doubles = d.off_b0 + work;
     d.tab_bytes = ((2 * 2 * d.zrec + 4 * 32) + 15) & ~15;   // rank16, recSQ (ground set Q), lvlZ
+    d.smem_bytes = (size_t)d.tab_bytes + sizeof(double) * (size_t)(d.off_stage + C * n * n + C * n);
+    return d;
+}
+
+// Orders 14..16: Z, the frontier and the reduction arrays live in a per-CTA block of global scratch (L2 resident
+// where it fits); W, the couplings, the tables and the staging buffer stay in shared memory.  Offsets are the same
+// in both spaces (the W part of the scratch block is simply unused).
+template <int C>
+inline PairDims pair_dims_global(int n, int threads)
+{
+    PairDims d = pair_dims<C>(n, 1);
+    d.threads = threads;
+    d.pslots = threads / (2 * C);
+    d.off_stage = d.off_z;                                // shared memory: W, -u, then the staging buffer
     d.smem_bytes = (size_t)d.tab_bytes + sizeof(double) * (size_t)(d.off_stage + C * n * n + C * n);
     return d;
 }
@@ -139,30 +155,34 @@ __device__ __forceinline__ void pair_store_rec(double* sm, int rec, double a0, d
 // diverges); an item with fewer targets pads with dummy columns that read a valid W column and are never stored.
 template <int C, int NC>
 __device__ __forceinline__ void pair_item(const PairLevel& L, unsigned SQ, int x, int u, double* sm, const double* Wl,
-                                          unsigned lanes)
+                                          unsigned lanes, int kskip = 0, bool last = true)
 {
     constexpr int WE = PairLayout<C>::WE, B = kPairB, N = NC - 1;
     const int n = L.n;
     const int q = 31 - __clz((int)SQ);
     const unsigned RQ = SQ ^ (1u << q);
     const int h = q + B;
-    int colo[NC];                     // W column offset of column k; the last one is the close column h
-    int orec[N > 0 ? N : 1];          // record number of target k in the next buffer
+    // Column window: Q-targets kskip, kskip + 1, .. of this pattern; in the LAST window of a pattern the final
+    // column is the close (column h).  Patterns with more columns than the register tile holds are processed in
+    // two windows (orders >= 14), each re-reading the sources.
+    int colo[NC];                     // W column offset of column k
+    int orec[NC];                     // record number of target k in the next buffer (-1: dummy / close)
     {
         unsigned absent = ~RQ & ((1u << q) - 1u);
+        for (int i = 0; i < kskip; ++i) absent &= absent - 1;
+        const int NQ = last ? N : NC;
 #pragma unroll
-        for (int k = 0; k < N; ++k) {
-            if (absent) {
+        for (int k = 0; k < NC; ++k) {
+            if (k < NQ && absent) {
                 const int d = __ffs(absent) - 1;
                 absent &= absent - 1;
                 colo[k] = (d + B) * WE;
                 orec[k] = __popc(RQ & ((1u << d) - 1u)) * L.cnt_next + L.rank16[SQ | (1u << d)];
             } else {
-                colo[k] = h * WE;      // dummy column
+                colo[k] = h * WE;      // dummy column, or the close
                 orec[k] = -1;
             }
         }
-        colo[N] = h * WE;
     }
     const int rowstride = n * WE;
     double acc[4][NC];
@@ -236,11 +256,24 @@ __device__ __forceinline__ void pair_item(const PairLevel& L, unsigned SQ, int x
     }
     // ---- outputs: next-level records, and Z[(SQ, R_T)] = -close (one -1 per closed fermion loop) ----
 #pragma unroll
-    for (int k = 0; k < N; ++k) {
+    for (int k = 0; k < NC; ++k) {
         if (orec[k] < 0) continue;
         pair_store_rec<C>(sm + L.off_nxt, orec[k], acc[0][k], acc[1][k], acc[2][k], acc[3][k]);
     }
-    pair_store_rec<C>(sm + L.off_z, L.lvlZ_j1 + x, -acc[0][N], -acc[1][N], -acc[2][N], -acc[3][N]);
+    if (last) pair_store_rec<C>(sm + L.off_z, L.lvlZ_j1 + x, -acc[0][N], -acc[1][N], -acc[2][N], -acc[3][N]);
+}
+
+template <int C, int NCMAX>
+__device__ __forceinline__ void pair_item_switch(int ncols, const PairLevel& L, unsigned SQ, int x, int u, double* sm,
+                                                 const double* Wl, unsigned lanes, int kskip, bool last)
+{
+#define COS_PAIR_CASE(K) case K: if (K <= NCMAX) { pair_item<C, (K <= NCMAX ? K : 1)>(L, SQ, x, u, sm, Wl, lanes, kskip, last); break; }
+    switch (ncols) {
+        COS_PAIR_CASE(1) COS_PAIR_CASE(2) COS_PAIR_CASE(3) COS_PAIR_CASE(4) COS_PAIR_CASE(5)
+        COS_PAIR_CASE(6) COS_PAIR_CASE(7) COS_PAIR_CASE(8) COS_PAIR_CASE(9)
+        default: pair_item<C, NCMAX>(L, SQ, x, u, sm, Wl, lanes, kskip, last); break;
+    }
+#undef COS_PAIR_CASE
 }
 
 template <int C, int MAXNC>
@@ -253,13 +286,12 @@ __device__ __forceinline__ void pair_dispatch_item(const PairLevel& L, unsigned 
     // both lanes of a pair are active together, so the shuffles inside an item see their partner
     const unsigned lanes = __ballot_sync(0xffffffffu, active);
     if (!active) return;
-#define COS_PAIR_CASE(K) case K - 1: if (K <= MAXNC) { pair_item<C, (K <= MAXNC ? K : 1)>(L, SQ, x, u, sm, Wl, lanes); break; }
-    switch (N) {
-        COS_PAIR_CASE(1) COS_PAIR_CASE(2) COS_PAIR_CASE(3) COS_PAIR_CASE(4) COS_PAIR_CASE(5)
-        COS_PAIR_CASE(6) COS_PAIR_CASE(7) COS_PAIR_CASE(8) COS_PAIR_CASE(9)
-        default: pair_item<C, MAXNC>(L, SQ, x, u, sm, Wl, lanes); break;
+    if (N + 1 <= MAXNC) {
+        pair_item_switch<C, MAXNC>(N + 1, L, SQ, x, u, sm, Wl, lanes, 0, true);
+    } else {                                   // two column windows: MAXNC Q-targets, then the rest and the close
+        pair_item<C, MAXNC>(L, SQ, x, u, sm, Wl, lanes, 0, false);
+        pair_item_switch<C, MAXNC>(N + 1 - MAXNC, L, SQ, x, u, sm, Wl, lanes, MAXNC, true);
     }
-#undef COS_PAIR_CASE
 }
 
 // Z[(SQ = {}, R_T)] for the 8 subsets of T (stages h < 3), one thread per instance, in the propagation's own
@@ -295,13 +327,13 @@ __device__ __forceinline__ void pair_small_stages(const double* Wl, int n, doubl
 // values R_T of record S_Q are the lo-values (S_Q & 3) * 4 + {0..3} of row hi = S_Q >> 2 in both arrays.
 // un[v * NC + cg] = -u_v of configuration cg (aliased species only; otherwise -u is folded into W).
 template <int C, int NC>
-__device__ __forceinline__ void pair_combine(double* smd, const PairDims& d, int ncfg, const uint16_t* recSQ,
-                                             int tid, int nthreads)
+__device__ __forceinline__ void pair_combine(double* smd, double* rb, const PairDims& d, int ncfg,
+                                             const uint16_t* recSQ, int tid, int nthreads)
 {
     using R = RedLayout<NC>;
     constexpr int NSP = C / NC;
-    double* CB = smd + d.off_cb;
-    double* DB = smd + d.off_db;
+    double* CB = rb + d.off_cb;
+    double* DB = rb + d.off_db;
     const double* un = smd + d.off_u;
     const int cg = tid % NC;
     if (cg >= ncfg) return;
@@ -320,8 +352,8 @@ __device__ __forceinline__ void pair_combine(double* smd, const PairDims& d, int
             unsigned m = SQ;
             while (m) { const int v = __ffs(m) - 1; m &= m - 1; wq *= un[(v + kPairB) * NC + cg]; }
         }
-        const double* zup = smd + d.off_z + (cg * NSP) * 4;
-        const double* zdn = smd + d.off_z + (cg * NSP + NSP - 1) * 4;
+        const double* zup = rb + d.off_z + (cg * NSP) * 4;
+        const double* zdn = rb + d.off_z + (cg * NSP + NSP - 1) * 4;
         double val[8];
 #pragma unroll
         for (int pi = 0; pi < 4; ++pi) {                  // values t = 2 pi, 2 pi + 1: lane half pi >> 1, chunk pi & 1
@@ -342,7 +374,7 @@ __device__ __forceinline__ void pair_combine(double* smd, const PairDims& d, int
     }
 }
 
-template <int C, int MAXT, int MINB, int MAXNC>
+template <int C, int MAXT, int MINB, int MAXNC, bool GLOBAL = false>
 __global__ void __launch_bounds__(MAXT, MINB) eval_pair_kernel(EvalArgs a, PairDims d)
 {
     using Lay = PairLayout<C>;
@@ -358,6 +390,7 @@ __global__ void __launch_bounds__(MAXT, MINB) eval_pair_kernel(EvalArgs a, PairD
     const uint16_t* mask16 = recSQ;
     const int* lvlT = lvlZ;
     double* smd = reinterpret_cast<double*>(smem_raw + d.tab_bytes);
+    double* rb = GLOBAL ? a.scratch + (size_t)blockIdx.x * a.scratch_stride : smd;   // record space
     const int tid = threadIdx.x, nthreads = blockDim.x;
     const int n = d.n, qmax = d.qmax, nsp = d.nsp;
     const unsigned NS = 1u << n;
@@ -365,7 +398,7 @@ __global__ void __launch_bounds__(MAXT, MINB) eval_pair_kernel(EvalArgs a, PairD
     const int g = (tid >> 1) % C;                // instance of this thread
     const int slot = tid / (2 * C);              // pattern slot
     const int rep = slot % REP;                  // W replica read by this thread
-    double* sm = smd + (2 * g + u) * 2;
+    double* sm = rb + (2 * g + u) * 2;
     const double* Wl = smd + d.off_w + rep * C + g;
 
     // the first team's inputs are fetched while the tables are being built
@@ -406,7 +439,7 @@ __global__ void __launch_bounds__(MAXT, MINB) eval_pair_kernel(EvalArgs a, PairD
             team_prefetch_inputs<C>(a, n, nsp, stage, nx0, (int)min((long long)C, total_inst - nx0), tid, nthreads);
         }
         COS_PHASE_MARK(0);
-        if (tid < ninst) pair_small_stages<C>(smd + d.off_w + tid, n, smd + d.off_z + tid * 4);
+        if (tid < ninst) pair_small_stages<C>(smd + d.off_w + tid, n, rb + d.off_z + tid * 4);
         __syncthreads();
         COS_PHASE_MARK(1);
 
@@ -433,7 +466,7 @@ __global__ void __launch_bounds__(MAXT, MINB) eval_pair_kernel(EvalArgs a, PairD
         // ---- a3 + a5 ("all"): D[full] = w * Zup[full] * Zdn[full]; S_Q = Q, R_T = T: lane half 1, chunk 1, e = 1 ----
         if (!a.connected) {
             if (tid < ncfg) {
-                const double* zp = smd + d.off_z + pair_chunk<C>(lvlZ[qmax], 1) + 2 + 1;
+                const double* zp = rb + d.off_z + pair_chunk<C>(lvlZ[qmax], 1) + 2 + 1;
                 const double zu = zp[(tid * nsp) * 4];
                 const double zd = zp[(tid * nsp + nsp - 1) * 4];
                 double w = 1.0;
@@ -444,17 +477,17 @@ __global__ void __launch_bounds__(MAXT, MINB) eval_pair_kernel(EvalArgs a, PairD
         }
 
         // ---- a3: combine, a4: connected reduction, a5: C'[full] ----
-        double* CB = smd + d.off_cb;
-        double* DB = smd + d.off_db;
+        double* CB = rb + d.off_cb;
+        double* DB = rb + d.off_db;
         if (nsp == 1) {
-            pair_combine<C, C>(smd, d, ncfg, recSQ, tid, nthreads);
+            pair_combine<C, C>(smd, rb, d, ncfg, recSQ, tid, nthreads);
             __syncthreads();
             COS_PHASE_MARK(12);
             team_reduce<C>(CB, DB, ncfg, n, mask16, lvlT, tid, nthreads);
             COS_PHASE_MARK(13);
             if (tid < ncfg) a.out[cfgbase + tid] = CB[red_elem<C>((NS >> (1 + kRedLB)) - 1, 15u, tid)];
         } else if constexpr (C >= 2) {
-            pair_combine<C, C / 2>(smd, d, ncfg, recSQ, tid, nthreads);
+            pair_combine<C, C / 2>(smd, rb, d, ncfg, recSQ, tid, nthreads);
             __syncthreads();
             COS_PHASE_MARK(12);
             team_reduce<C / 2>(CB, DB, ncfg, n, mask16, lvlT, tid, nthreads);
