@@ -153,10 +153,12 @@ __device__ __forceinline__ void pair_store_rec(double* sm, int rec, double a0, d
 // NC = N + 1 columns are accumulated in registers: the N = q - j Q-targets and the close (column h), together
 // with the 8 T-target accumulators.  NC is the widest item of the WARP (warp-uniform, the dispatch never
 // diverges); an item with fewer targets pads with dummy columns that read a valid W column and are never stored.
-template <int C, int NC>
+template <int C, int NC, int KSKIP = 0, bool LAST = true>
 __device__ __forceinline__ void pair_item(const PairLevel& L, unsigned SQ, int x, int u, double* sm, const double* Wl,
-                                          unsigned lanes, int kskip = 0, bool last = true)
+                                          unsigned lanes)
 {
+    constexpr int kskip = KSKIP;
+    constexpr bool last = LAST;
     constexpr int WE = PairLayout<C>::WE, B = kPairB, N = NC - 1;
     const int n = L.n;
     const int q = 31 - __clz((int)SQ);
@@ -263,20 +265,21 @@ __device__ __forceinline__ void pair_item(const PairLevel& L, unsigned SQ, int x
     if (last) pair_store_rec<C>(sm + L.off_z, L.lvlZ_j1 + x, -acc[0][N], -acc[1][N], -acc[2][N], -acc[3][N]);
 }
 
-template <int C, int NCMAX>
+template <int C, int NCMAX, int KSKIP>
 __device__ __forceinline__ void pair_item_switch(int ncols, const PairLevel& L, unsigned SQ, int x, int u, double* sm,
-                                                 const double* Wl, unsigned lanes, int kskip, bool last)
+                                                 const double* Wl, unsigned lanes)
 {
-#define COS_PAIR_CASE(K) case K: if (K <= NCMAX) { pair_item<C, (K <= NCMAX ? K : 1)>(L, SQ, x, u, sm, Wl, lanes, kskip, last); break; }
+#define COS_PAIR_CASE(K) case K: if (K <= NCMAX) { pair_item<C, (K <= NCMAX ? K : 1), KSKIP, true>(L, SQ, x, u, sm, Wl, lanes); break; }
     switch (ncols) {
         COS_PAIR_CASE(1) COS_PAIR_CASE(2) COS_PAIR_CASE(3) COS_PAIR_CASE(4) COS_PAIR_CASE(5)
         COS_PAIR_CASE(6) COS_PAIR_CASE(7) COS_PAIR_CASE(8) COS_PAIR_CASE(9)
-        default: pair_item<C, NCMAX>(L, SQ, x, u, sm, Wl, lanes, kskip, last); break;
+        default: pair_item<C, NCMAX, KSKIP, true>(L, SQ, x, u, sm, Wl, lanes); break;
     }
 #undef COS_PAIR_CASE
 }
 
-template <int C, int MAXNC>
+// WINDOWS: patterns may have more columns than MAXNC (orders >= 14) and are then processed in two column windows.
+template <int C, int MAXNC, bool WINDOWS>
 __device__ __forceinline__ void pair_dispatch_item(const PairLevel& L, unsigned SQ, int x, int u, double* sm,
                                                    const double* Wl, bool active)
 {
@@ -286,11 +289,11 @@ __device__ __forceinline__ void pair_dispatch_item(const PairLevel& L, unsigned 
     // both lanes of a pair are active together, so the shuffles inside an item see their partner
     const unsigned lanes = __ballot_sync(0xffffffffu, active);
     if (!active) return;
-    if (N + 1 <= MAXNC) {
-        pair_item_switch<C, MAXNC>(N + 1, L, SQ, x, u, sm, Wl, lanes, 0, true);
-    } else {                                   // two column windows: MAXNC Q-targets, then the rest and the close
-        pair_item<C, MAXNC>(L, SQ, x, u, sm, Wl, lanes, 0, false);
-        pair_item_switch<C, MAXNC>(N + 1 - MAXNC, L, SQ, x, u, sm, Wl, lanes, MAXNC, true);
+    if (!WINDOWS || N + 1 <= MAXNC) {
+        pair_item_switch<C, MAXNC, 0>(N + 1, L, SQ, x, u, sm, Wl, lanes);
+    } else if constexpr (WINDOWS) {            // MAXNC Q-targets, then the rest and the close
+        pair_item<C, MAXNC, 0, false>(L, SQ, x, u, sm, Wl, lanes);
+        pair_item_switch<C, MAXNC, MAXNC>(N + 1 - MAXNC, L, SQ, x, u, sm, Wl, lanes);
     }
 }
 
@@ -457,7 +460,7 @@ __global__ void __launch_bounds__(MAXT, MINB) eval_pair_kernel(EvalArgs a, PairD
             for (int x0 = 0; x0 < L.cnt; x0 += d.pslots) {
                 const int x = x0 + slot;
                 const bool active = (x < L.cnt) && (g < ninst);
-                pair_dispatch_item<C, MAXNC>(L, active ? masks[x] : 1u, x, u, sm, Wl, active);
+                pair_dispatch_item<C, MAXNC, GLOBAL>(L, active ? masks[x] : 1u, x, u, sm, Wl, active);
             }
             __syncthreads();
             COS_PHASE_MARK(2 + j);
