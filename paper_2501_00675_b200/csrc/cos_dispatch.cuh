@@ -107,11 +107,11 @@ inline PairChoice pair_choice(int n, int nsp)
 inline bool has_fused_kernel(int, int, int) { return false; }
 
 // ---- pair kernel on global records (orders 14..16, one species): Z / frontier / reduction arrays in L2 scratch ----
-constexpr int kPairGlobalMinN = 14, kPairGlobalThreads = 256;
+constexpr int kPairGlobalMinN = 14, kPairGlobalThreads = 512;
 inline bool uses_pair_global(int n, int nsp) { return n >= kPairGlobalMinN && n <= kMaxN && nsp == 1; }
 inline PairChoice pair_global_choice(int n)
 {
-    return {eval_pair_kernel<1, kPairGlobalThreads, 2, 8, true>, pair_dims_global<1>(n, kPairGlobalThreads)};
+    return {eval_pair_kernel<1, kPairGlobalThreads, 1, 8, true>, pair_dims_global<1>(n, kPairGlobalThreads)};
 }
 inline size_t pair_global_rec_doubles(int n)
 {
