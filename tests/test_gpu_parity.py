@@ -202,3 +202,34 @@ def test_probes_report_plausible_peaks(ctx):
     print(f"DFMA probe {tf:.2f} TFLOP/s, shared-memory probe {bw:.0f} GB/s")
     assert 10.0 < tf < 80.0
     assert 5e3 < bw < 1e5
+
+
+# ------------------------------------------------------------------------------------------ full sizes
+@pytest.mark.parametrize("cfg,nsample", [(2, 512), (3, 512), (4, 128), (5, 8)])
+def test_full_size_sampled_outputs(torch_mod, oracle_mod, cfg, nsample):
+    """BASELINE.json configs at their FULL batch, through the entry point and launch configuration bench.py
+    times (cos_eval_connected_xt for the Hubbard configs: build_G + evaluation over the whole batch;
+    cos_eval_connected for config 5), checked on a seeded sample of outputs the oracle computes one by one."""
+    from paper_2501_00675_b200 import api, workloads as wl
+    torch = torch_mod
+    w = wl.baseline_config(cfg)                       # full batch: 4096 / 16384 / 4096 / 512
+    out = torch.empty(w.batch, dtype=torch.float64, device="cuda")
+    with api.Context() as c:
+        if w.kind == "hubbard":
+            c.set_g0_table(_dev(torch, w.table), w.beta)
+            c.eval_connected_xt(_dev(torch, w.xy), _dev(torch, w.tau), out, U=w.U, g_diag=w.g_diag)
+        else:
+            dG = _dev(torch, w.G)
+            c.eval_connected(dG, dG, out, U=w.U, d_u=_dev(torch, w.u))
+        torch.cuda.synchronize()
+        assert c.last_launch_count() >= 1
+    got = out.cpu().numpy()
+    assert np.all(np.isfinite(got))
+    idx = np.sort(np.random.default_rng(77 + cfg).choice(w.batch, size=min(nsample, w.batch), replace=False))
+    idx[0], idx[-1] = 0, w.batch - 1                  # first and last configuration of the batch (ragged last team)
+    if w.kind == "hubbard":
+        Gup, _ = oracle_mod.build_G(w.xy[idx], w.tau[idx], w.table, None, w.beta, w.g_diag)
+        check_parity(oracle_mod, got[idx], Gup, None, w.U, None, "connected")
+    else:
+        check_parity(oracle_mod, got[idx], np.ascontiguousarray(w.G[idx]), None, w.U,
+                     np.ascontiguousarray(w.u[idx]), "connected")
