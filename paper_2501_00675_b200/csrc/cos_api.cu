@@ -25,7 +25,8 @@ struct cos_ctx {
     // scratch (owned)
     uint32_t* off = nullptr;
     double* scratch = nullptr;      size_t scratch_bytes = 0;
-    double* gscratch = nullptr;     size_t gscratch_bytes = 0;   // G matrices of the fused path
+    double* gscratch = nullptr;     size_t gscratch_bytes = 0;   // G matrices of cos_eval_connected_xt
+    unsigned char* team_tabs[COS_MAX_ORDER + 1] = {};            // table images of the team kernel, by order
     void* stage = nullptr;          size_t stage_bytes = 0;      // device staging of the host path
     // bookkeeping
     int last_launches = 0;
@@ -113,6 +114,17 @@ int do_eval(cos_ctx* c, int n, long long batch, const double* gup, const double*
     EvalArgs a{};
     a.n = n; a.batch = batch; a.Gup = gup; a.Gdn = gdn; a.u = u; a.U = U; a.out = out;
     a.connected = connected; a.off = c->off;
+    if (uses_team(n)) {          // table image of this order, built on first use
+        if (!c->team_tabs[n]) {
+            const TeamDims td = team_choice(n, 1).d;
+            unsigned char* buf = nullptr;
+            if (cudaMalloc((void**)&buf, (size_t)td.tab_bytes) != cudaSuccess) return COS_ENOMEM;
+            team_tables_kernel<<<1, 256, (size_t)td.tab_bytes, c->stream>>>(td, buf);
+            COS_CUDA(c, cudaGetLastError());
+            c->team_tabs[n] = buf;
+        }
+        a.tabs = c->team_tabs[n];
+    }
     // global scratch for the orders whose frontier does not fit in shared memory
     const size_t per_cta = eval_scratch_doubles(n, c->smem_optin);
     if (per_cta) {
@@ -218,6 +230,7 @@ int cos_destroy(cos_ctx* c)
     cudaFree(c->scratch);
     cudaFree(c->gscratch);
     cudaFree(c->stage);
+    for (int i = 0; i <= COS_MAX_ORDER; ++i) cudaFree(c->team_tabs[i]);
     delete c;
     return COS_OK;
 }

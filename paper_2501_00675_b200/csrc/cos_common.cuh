@@ -37,7 +37,8 @@ struct EvalArgs {
     const uint32_t* off;   // off[R] = sum_{x<R}(popc(x)+1), R = 0..2^(kMaxN-1)
     double* scratch;       // per-CTA global scratch (large n), may be nullptr
     size_t scratch_stride; // doubles per CTA
-    int fused;             // 1: matrices are assembled on the fly from bg (Gup/Gdn unused); team kernel only
+    int fused;             // unused (no kernel assembles G on the fly any more); kept 0
+    const unsigned char* tabs;   // team kernel: table image of this order built once per context (or nullptr)
     BuildGArgs bg;
 };
 

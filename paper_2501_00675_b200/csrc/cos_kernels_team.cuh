@@ -780,6 +780,62 @@ __device__ __forceinline__ void team_unpack_inputs(const EvalArgs& a, int n, int
         }
 }
 
+// All per-order tables of the team kernel, into the table area at the start of shared memory (layout: TeamDims).
+__device__ __forceinline__ void team_build_tables(unsigned char* smem_raw, const TeamDims& d, int tid, int nthreads)
+{
+    const int n = d.n, qmax = d.qmax;
+    uint16_t* mask16 = reinterpret_cast<uint16_t*>(smem_raw);
+    uint16_t* rank16 = mask16 + (1 << (d.n - 1));
+    int* lvlT = reinterpret_cast<int*>(rank16 + (1 << (d.n - 1)));
+    int* lvlZ = lvlT + 32;
+    uint16_t* recSQ = reinterpret_cast<uint16_t*>(lvlZ + 32);
+    // ---- tables: subsets of {0..n-2} by popcount in colex order (rank independent of the ground set) ----
+    if (tid == 0) {
+        int run = 0;
+        for (int j = 0; j <= n; ++j) { lvlT[j] = run; run += kBinom.c[n - 1][j]; }
+        run = 0;
+        for (int j = 0; j <= qmax + 1; ++j) { lvlZ[j] = run; run += kBinom.c[qmax][j]; }
+    }
+    __syncthreads();
+    for (unsigned mk = tid; mk < (1u << (n - 1)); mk += nthreads) {
+        int rk = 0, i = 0;
+        unsigned m = mk;
+        while (m) { const int s = __ffs(m) - 1; m &= m - 1; ++i; rk += kBinom.c[s][i]; }
+        rank16[mk] = (uint16_t)rk;
+        mask16[lvlT[i] + rk] = (uint16_t)mk;
+        if (mk < (1u << qmax)) recSQ[lvlZ[i] + rk] = (uint16_t)mk;
+    }
+    __syncthreads();
+    uint32_t* dtab = reinterpret_cast<uint32_t*>(smem_raw + d.dsc_off);
+    for (int r = 1 + tid; r < (1 << qmax); r += nthreads) team_build_descriptor(dtab + r * 8, recSQ[r], qmax, lvlZ, rank16);
+    // column units (pattern x | column << 8) of level 0, their count in ucol[254]
+    uint16_t* ucol = reinterpret_cast<uint16_t*>(smem_raw + d.dsc_off + 32 * d.zrec);
+    __syncthreads();
+    if (tid == 0) {
+        int u = 0;
+        for (int j = 0; j < 1; ++j) {
+            for (int x = 0; x < kBinom.c[qmax][j + 1]; ++x) {
+                const int nown = (int)(dtab[(lvlZ[j + 1] + x) * 8 + 4] >> 28);
+                for (int k = 0; k <= nown && u < 254; ++k) ucol[u++] = (uint16_t)(x | (k << 8));
+            }
+            ucol[254 + j] = (uint16_t)u;
+        }
+    }
+
+    __syncthreads();
+}
+
+// Builds the table image of one order once (one CTA); the evaluation kernels copy it instead of rebuilding it
+// per CTA (the construction costs about 12 k cycles, a quarter of a whole order-8 launch at batch 4096).
+__global__ void __launch_bounds__(256) team_tables_kernel(TeamDims d, unsigned char* out)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    team_build_tables(smem_raw, d, threadIdx.x, blockDim.x);
+    const uint4* src = reinterpret_cast<const uint4*>(smem_raw);
+    uint4* dst = reinterpret_cast<uint4*>(out);
+    for (int i = threadIdx.x; i < d.tab_bytes / 16; i += blockDim.x) dst[i] = src[i];
+}
+
 // Team kernel: the next team's matrices go straight into the replicated W with cp.async, issued as soon as the
 // last propagation level has released W (the combine and the reduction do not read it), so that a team starts with
 // its W in place -- no staging pass.  Only the couplings (a few values) are staged.
@@ -872,37 +928,16 @@ __global__ void __launch_bounds__(MAXT, MINB) eval_team_kernel(EvalArgs a, TeamD
         const long long nx0 = (long long)blockIdx.x * C;
         team_prefetch_w<C, REP>(a, n, nsp, smd + d.off_w, stage, nx0, (int)min((long long)C, total_inst - nx0), tid, nthreads);
     }
-    // ---- tables: subsets of {0..n-2} by popcount in colex order (rank independent of the ground set) ----
-    if (tid == 0) {
-        int run = 0;
-        for (int j = 0; j <= n; ++j) { lvlT[j] = run; run += kBinom.c[n - 1][j]; }
-        run = 0;
-        for (int j = 0; j <= qmax + 1; ++j) { lvlZ[j] = run; run += kBinom.c[qmax][j]; }
-    }
-    team_sync(nthreads);
-    for (unsigned mk = tid; mk < (1u << (n - 1)); mk += nthreads) {
-        int rk = 0, i = 0;
-        unsigned m = mk;
-        while (m) { const int s = __ffs(m) - 1; m &= m - 1; ++i; rk += kBinom.c[s][i]; }
-        rank16[mk] = (uint16_t)rk;
-        mask16[lvlT[i] + rk] = (uint16_t)mk;
-        if (mk < (1u << qmax)) recSQ[lvlZ[i] + rk] = (uint16_t)mk;
-    }
-    __syncthreads();
+    // ---- tables (subset lists, ranks, item descriptors, column units): copied from the image the context built
+    //      once per order (team_tables_kernel), or built here when no image is given ----
     uint32_t* dtab = reinterpret_cast<uint32_t*>(smem_raw + d.dsc_off);
-    for (int r = 1 + tid; r < (1 << qmax); r += nthreads) team_build_descriptor(dtab + r * 8, recSQ[r], qmax, lvlZ, rank16);
-    // column units (pattern x | column << 8) of level 0, their count in ucol[254]
     uint16_t* ucol = reinterpret_cast<uint16_t*>(smem_raw + d.dsc_off + 32 * d.zrec);
-    __syncthreads();
-    if (tid == 0) {
-        int u = 0;
-        for (int j = 0; j < 1; ++j) {
-            for (int x = 0; x < kBinom.c[qmax][j + 1]; ++x) {
-                const int nown = (int)(dtab[(lvlZ[j + 1] + x) * 8 + 4] >> 28);
-                for (int k = 0; k <= nown && u < 254; ++k) ucol[u++] = (uint16_t)(x | (k << 8));
-            }
-            ucol[254 + j] = (uint16_t)u;
-        }
+    if (a.tabs != nullptr) {
+        const uint4* src = reinterpret_cast<const uint4*>(a.tabs);
+        uint4* dst = reinterpret_cast<uint4*>(smem_raw);
+        for (int i = tid; i < d.tab_bytes / 16; i += nthreads) dst[i] = __ldg(src + i);
+    } else {
+        team_build_tables(smem_raw, d, tid, nthreads);
     }
 
     const bool col_ok = qmax >= 2 && qmax <= 7;      // unit table: 28 + 91 entries at most (order 10)
