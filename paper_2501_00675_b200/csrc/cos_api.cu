@@ -26,7 +26,8 @@ struct cos_ctx {
     uint32_t* off = nullptr;
     double* scratch = nullptr;      size_t scratch_bytes = 0;
     double* gscratch = nullptr;     size_t gscratch_bytes = 0;   // G matrices of cos_eval_connected_xt
-    unsigned char* team_tabs[COS_MAX_ORDER + 1] = {};            // table images of the team kernel, by order
+    unsigned char* team_tabs[COS_MAX_ORDER + 1] = {};            // per order: table image of the team kernel / item
+                                                                 // descriptors of the pair kernel
     void* stage = nullptr;          size_t stage_bytes = 0;      // device staging of the host path
     // bookkeeping
     int last_launches = 0;
@@ -120,6 +121,16 @@ int do_eval(cos_ctx* c, int n, long long batch, const double* gup, const double*
             unsigned char* buf = nullptr;
             if (cudaMalloc((void**)&buf, (size_t)td.tab_bytes) != cudaSuccess) return COS_ENOMEM;
             team_tables_kernel<<<1, 256, (size_t)td.tab_bytes, c->stream>>>(td, buf);
+            COS_CUDA(c, cudaGetLastError());
+            c->team_tabs[n] = buf;
+        }
+        a.tabs = c->team_tabs[n];
+    } else if (n >= kPairGlobalMinN) {   // item descriptors of the global-record pair kernel, built on first use
+        if (!c->team_tabs[n]) {
+            const size_t bytes = ((size_t)1 << (n - kPairB)) * kPairDscWords * sizeof(uint32_t);
+            unsigned char* buf = nullptr;
+            if (cudaMalloc((void**)&buf, bytes) != cudaSuccess) return COS_ENOMEM;
+            pair_tables_kernel<<<32, 256, 0, c->stream>>>(n, reinterpret_cast<uint32_t*>(buf));
             COS_CUDA(c, cudaGetLastError());
             c->team_tabs[n] = buf;
         }

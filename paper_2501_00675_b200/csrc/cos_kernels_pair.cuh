@@ -129,7 +129,54 @@ struct PairLevel {
     int lvlZ_j, lvlZ_j1;        // Z record offsets of |S_Q| = j and j + 1
     int off_z, off_cur, off_nxt;
     const uint16_t* rank16;
+    const uint32_t* dsc;        // item descriptors (12 words per pattern, indexed by the Z record of S_Q), global memory
 };
+
+// ---- item descriptors of the pair kernel: one 48-byte record per Q-pattern, built once per order into global
+//      memory by pair_tables_kernel (the table does not fit beside the frontier in shared memory; it is read
+//      through L1).  An item's prologue is three 16-byte loads instead of a chain of bit tricks and rank look-ups.
+//   w0: Z record of S_Q \ {top} | h << 16 | number of Q-targets << 24
+//   w1, w2: column vertices of the Q-targets (4 bits each, ascending)     w3, w4: source vertices (4 bits each)
+//   w5..w11: record numbers of the Q-targets in the next level buffer (16 bits each)
+constexpr int kPairDscWords = 12;
+
+__device__ __forceinline__ int colex_rank(unsigned m)
+{
+    int rk = 0, i = 0;
+    while (m) { const int s = __ffs(m) - 1; m &= m - 1; ++i; rk += kBinom.c[s][i]; }
+    return rk;
+}
+
+__global__ void __launch_bounds__(256) pair_tables_kernel(int n, uint32_t* out)
+{
+    const int qmax = n - kPairB;
+    for (unsigned SQ = 1 + blockIdx.x * blockDim.x + threadIdx.x; SQ < (1u << qmax); SQ += gridDim.x * blockDim.x) {
+        const int j = __popc(SQ) - 1;
+        const int q = 31 - __clz((int)SQ);
+        const unsigned RQ = SQ ^ (1u << q);
+        int lvlZ_j = 0, lvlZ_j1 = 0;
+        for (int i = 0; i <= j; ++i) { if (i < j) lvlZ_j += kBinom.c[qmax][i]; lvlZ_j1 += kBinom.c[qmax][i]; }
+        const int cnt_next = kBinom.c[qmax][j + 2];
+        uint32_t w[kPairDscWords];
+#pragma unroll
+        for (int i = 0; i < kPairDscWords; ++i) w[i] = 0;
+        unsigned absent = ~RQ & ((1u << q) - 1u);
+        int k = 0;
+        for (; absent; ++k) {
+            const int d = __ffs(absent) - 1;
+            absent &= absent - 1;
+            const uint32_t orec = (uint32_t)(__popc(RQ & ((1u << d) - 1u)) * cnt_next + colex_rank(SQ | (1u << d)));
+            w[1 + (k >> 3)] |= (uint32_t)(d + kPairB) << (4 * (k & 7));
+            w[5 + (k >> 1)] |= orec << (16 * (k & 1));
+        }
+        w[0] = (uint32_t)(lvlZ_j + colex_rank(RQ)) | ((uint32_t)(q + kPairB) << 16) | ((uint32_t)k << 24);
+        unsigned m = RQ;
+        for (int i = 0; m; ++i) { const int v = __ffs(m) - 1 + kPairB; m &= m - 1; w[3 + (i >> 3)] |= (uint32_t)v << (4 * (i & 7)); }
+        uint32_t* dst = out + (size_t)(lvlZ_j1 + colex_rank(SQ)) * kPairDscWords;
+#pragma unroll
+        for (int i = 0; i < kPairDscWords; ++i) dst[i] = w[i];
+    }
+}
 
 // The 4 values (rows r = 0..3 of this lane half) of record rec.  sm already carries the lane part.
 template <int C>
@@ -153,7 +200,7 @@ __device__ __forceinline__ void pair_store_rec(double* sm, int rec, double a0, d
 // NC = N + 1 columns are accumulated in registers: the N = q - j Q-targets and the close (column h), together
 // with the 8 T-target accumulators.  NC is the widest item of the WARP (warp-uniform, the dispatch never
 // diverges); an item with fewer targets pads with dummy columns that read a valid W column and are never stored.
-template <int C, int NC, int KSKIP = 0, bool LAST = true>
+template <int C, int NC, int KSKIP = 0, bool LAST = true, bool DSC = false>
 __device__ __forceinline__ void pair_item(const PairLevel& L, unsigned SQ, int x, int u, double* sm, const double* Wl,
                                           unsigned lanes)
 {
@@ -161,18 +208,42 @@ __device__ __forceinline__ void pair_item(const PairLevel& L, unsigned SQ, int x
     constexpr bool last = LAST;
     constexpr int WE = PairLayout<C>::WE, B = kPairB, N = NC - 1;
     const int n = L.n;
-    const int q = 31 - __clz((int)SQ);
-    const unsigned RQ = SQ ^ (1u << q);
-    const int h = q + B;
     // Column window: Q-targets kskip, kskip + 1, .. of this pattern; in the LAST window of a pattern the final
     // column is the close (column h).  Patterns with more columns than the register tile holds are processed in
     // two windows (orders >= 14), each re-reading the sources.
     int colo[NC];                     // W column offset of column k
     int orec[NC];                     // record number of target k in the next buffer (-1: dummy / close)
-    {
+    int zrec, h;
+    unsigned long long srcs;          // source vertices, 4 bits each
+    constexpr int NQ = last ? N : NC;
+    if constexpr (DSC) {
+        // prologue from the descriptor table (global-record variant: L1 is large there; for the shared-memory
+        // variants, whose L1 is a few KB, the table reads measured slower than the bit tricks below)
+        const uint4* dp = reinterpret_cast<const uint4*>(L.dsc + (size_t)(L.lvlZ_j1 + x) * kPairDscWords);
+        const uint4 d0 = __ldg(dp), d1 = __ldg(dp + 1), d2 = __ldg(dp + 2);
+        const uint32_t dw[kPairDscWords] = {d0.x, d0.y, d0.z, d0.w, d1.x, d1.y, d1.z, d1.w, d2.x, d2.y, d2.z, d2.w};
+        zrec = (int)(dw[0] & 0xffffu);
+        h = (int)((dw[0] >> 16) & 15u);
+        const int nown = (int)(dw[0] >> 24);
+#pragma unroll
+        for (int k = 0; k < NC; ++k) {
+            const int t = kskip + k;                       // target index (compile time after unrolling)
+            if (k < NQ && t < nown) {
+                colo[k] = (int)((dw[1 + (t >> 3)] >> (4 * (t & 7))) & 15u) * WE;
+                orec[k] = (int)((dw[5 + (t >> 1)] >> (16 * (t & 1))) & 0xffffu);
+            } else {
+                colo[k] = h * WE;      // dummy column, or the close
+                orec[k] = -1;
+            }
+        }
+        srcs = (unsigned long long)dw[3] | ((unsigned long long)dw[4] << 32);
+    } else {
+        const int q = 31 - __clz((int)SQ);
+        const unsigned RQ = SQ ^ (1u << q);
+        h = q + B;
+        zrec = L.lvlZ_j + L.rank16[RQ];
         unsigned absent = ~RQ & ((1u << q) - 1u);
         for (int i = 0; i < kskip; ++i) absent &= absent - 1;
-        const int NQ = last ? N : NC;
 #pragma unroll
         for (int k = 0; k < NC; ++k) {
             if (k < NQ && absent) {
@@ -185,6 +256,7 @@ __device__ __forceinline__ void pair_item(const PairLevel& L, unsigned SQ, int x
                 orec[k] = -1;
             }
         }
+        srcs = RQ;                     // the loop below peels the source vertices off this mask
     }
     const int rowstride = n * WE;
     double acc[4][NC];
@@ -192,7 +264,7 @@ __device__ __forceinline__ void pair_item(const PairLevel& L, unsigned SQ, int x
     // ---- the start node (S, h) = Z[S \ {h}] ("top node", one per stage) ----
     {
         double a[4];
-        pair_load_rec<C>(sm + L.off_z, L.lvlZ_j + L.rank16[RQ], a);
+        pair_load_rec<C>(sm + L.off_z, zrec, a);
         const double* row = Wl + h * rowstride;
 #pragma unroll
         for (int k = 0; k < NC; ++k) {
@@ -207,11 +279,11 @@ __device__ __forceinline__ void pair_item(const PairLevel& L, unsigned SQ, int x
     }
     // ---- sources in Q, streamed from the level buffer ----
     {
-        unsigned m = RQ;
         int rec = x;
         for (int i = 0; i < L.j; ++i) {
-            const int v = __ffs(m) - 1 + B;
-            m &= m - 1;
+            int v;
+            if constexpr (DSC) { v = (int)(srcs & 15u); srcs >>= 4; }
+            else { const unsigned mm = (unsigned)srcs; v = __ffs(mm) - 1 + B; srcs = mm & (mm - 1); }
             double a[4];
             pair_load_rec<C>(sm + L.off_cur, rec, a);
             rec += L.cnt;
@@ -265,15 +337,15 @@ __device__ __forceinline__ void pair_item(const PairLevel& L, unsigned SQ, int x
     if (last) pair_store_rec<C>(sm + L.off_z, L.lvlZ_j1 + x, -acc[0][N], -acc[1][N], -acc[2][N], -acc[3][N]);
 }
 
-template <int C, int NCMAX, int KSKIP>
+template <int C, int NCMAX, int KSKIP, bool DSC>
 __device__ __forceinline__ void pair_item_switch(int ncols, const PairLevel& L, unsigned SQ, int x, int u, double* sm,
                                                  const double* Wl, unsigned lanes)
 {
-#define COS_PAIR_CASE(K) case K: if (K <= NCMAX) { pair_item<C, (K <= NCMAX ? K : 1), KSKIP, true>(L, SQ, x, u, sm, Wl, lanes); break; }
+#define COS_PAIR_CASE(K) case K: if (K <= NCMAX) { pair_item<C, (K <= NCMAX ? K : 1), KSKIP, true, DSC>(L, SQ, x, u, sm, Wl, lanes); break; }
     switch (ncols) {
         COS_PAIR_CASE(1) COS_PAIR_CASE(2) COS_PAIR_CASE(3) COS_PAIR_CASE(4) COS_PAIR_CASE(5)
         COS_PAIR_CASE(6) COS_PAIR_CASE(7) COS_PAIR_CASE(8) COS_PAIR_CASE(9)
-        default: pair_item<C, NCMAX, KSKIP, true>(L, SQ, x, u, sm, Wl, lanes); break;
+        default: pair_item<C, NCMAX, KSKIP, true, DSC>(L, SQ, x, u, sm, Wl, lanes); break;
     }
 #undef COS_PAIR_CASE
 }
@@ -290,10 +362,10 @@ __device__ __forceinline__ void pair_dispatch_item(const PairLevel& L, unsigned 
     const unsigned lanes = __ballot_sync(0xffffffffu, active);
     if (!active) return;
     if (!WINDOWS || N + 1 <= MAXNC) {
-        pair_item_switch<C, MAXNC, 0>(N + 1, L, SQ, x, u, sm, Wl, lanes);
+        pair_item_switch<C, MAXNC, 0, WINDOWS>(N + 1, L, SQ, x, u, sm, Wl, lanes);
     } else if constexpr (WINDOWS) {            // MAXNC Q-targets, then the rest and the close
-        pair_item<C, MAXNC, 0, false>(L, SQ, x, u, sm, Wl, lanes);
-        pair_item_switch<C, MAXNC, MAXNC>(N + 1 - MAXNC, L, SQ, x, u, sm, Wl, lanes);
+        pair_item<C, MAXNC, 0, false, true>(L, SQ, x, u, sm, Wl, lanes);
+        pair_item_switch<C, MAXNC, MAXNC, true>(N + 1 - MAXNC, L, SQ, x, u, sm, Wl, lanes);
     }
 }
 
@@ -448,7 +520,7 @@ __global__ void __launch_bounds__(MAXT, MINB) eval_pair_kernel(EvalArgs a, PairD
 
         // ---- a2: all stages together, level j = |S_Q| - 1; level j reads buffer (j & 1) and writes the other ----
         PairLevel L;
-        L.n = n; L.rank16 = rank16; L.off_z = d.off_z;
+        L.n = n; L.rank16 = rank16; L.off_z = d.off_z; L.dsc = reinterpret_cast<const uint32_t*>(a.tabs);
         for (int j = 0; j < qmax; ++j) {
             L.j = j;
             L.cnt = kBinom.c[qmax][j + 1];
