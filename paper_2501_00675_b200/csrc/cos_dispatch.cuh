@@ -98,7 +98,7 @@ inline PairChoice pair_choice(int n, int nsp)
 {
     if (n == 13) return {eval_pair_kernel<1, 512, 1, 10>, pair_dims<1>(n, 1)};   // one species only (see dispatch_eval)
     if (n == 12) return {eval_pair_kernel<2, 512, 1, 9>, pair_dims<2>(n, nsp)};
-    return {eval_pair_kernel<4, 576, 1, 8>, pair_dims<4>(n, nsp)};
+    return {eval_pair_kernel<4, 512, 1, 8>, pair_dims<4>(n, nsp, 512)};
 }
 
 // No evaluation kernel assembles G on the fly any more: a separate cos_build_G launch plus a cp.async prefetch of

@@ -71,7 +71,7 @@ struct PairDims {
 };
 
 template <int C>
-inline PairDims pair_dims(int n, int nsp)
+inline PairDims pair_dims(int n, int nsp, int max_threads = 1024)
 {
     using L = PairLayout<C>;
     PairDims d{};
@@ -80,6 +80,7 @@ inline PairDims pair_dims(int n, int nsp)
     int slots = team_max_patterns(n);
     slots = (slots + L::PW - 1) / L::PW * L::PW;
     if (slots * 2 * C < 64) slots = 64 / (2 * C);
+    if (slots * 2 * C > max_threads) slots = max_threads / (2 * C);   // the widest levels then take two passes
     d.pslots = slots;
     d.threads = slots * 2 * C;
     int rec_even = 1, rec_odd = 1;                        // ping-pong buffers sized for the levels they hold
