@@ -94,7 +94,7 @@ inline PairDims pair_dims(int n, int nsp, int max_threads = 1024)
     d.red_rows = 1 << (n - 1 - kRedLB);
     d.off_w = 0;
     d.off_u = d.off_w + n * n * L::WE;
-    d.off_z = d.off_u + 16 * d.ncfg;                      // un[v][cfg] = -u_v
+    d.off_z = d.off_u + (16 + 192) * d.ncfg;              // un[v][cfg] = -u_v, then the 128 + 64 products of pair_combine
     d.off_b0 = d.off_z + d.zrec * L::REC;
     d.off_b1 = d.off_b0 + rec_even * L::REC;              // level j reads buffer (j & 1), writes buffer (~j & 1)
     int work = (rec_even + rec_odd) * L::REC;
@@ -412,6 +412,17 @@ __device__ __forceinline__ void pair_combine(double* smd, double* rb, const Pair
     double* DB = rb + d.off_db;
     const double* un = smd + d.off_u;
     const int cg = tid % NC;
+    // w(S_Q) = wt[S_Q & 127] * wt[128 + (S_Q >> 7)]: products over the 7 low / 6 high vertices of Q, once per team
+    double* wt = smd + d.off_u + 16 * NC;
+    if (NSP == 1) {
+        for (int t = tid / NC; t < 192; t += nthreads / NC) {
+            unsigned m = t < 128 ? (unsigned)t : (unsigned)(t - 128) << 7;
+            double w = 1.0;
+            while (m) { const int v = __ffs(m) - 1; m &= m - 1; if (v < d.qmax) w *= un[(v + kPairB) * NC + cg]; }
+            wt[t * NC + cg] = w;
+        }
+        __syncthreads();
+    }
     if (cg >= ncfg) return;
     double wT[8];
 #pragma unroll
@@ -423,11 +434,7 @@ __device__ __forceinline__ void pair_combine(double* smd, double* rb, const Pair
     }
     for (int rec = tid / NC; rec < d.zrec; rec += nthreads / NC) {
         const unsigned SQ = recSQ[rec];
-        double wq = 1.0;
-        if (NSP == 1) {
-            unsigned m = SQ;
-            while (m) { const int v = __ffs(m) - 1; m &= m - 1; wq *= un[(v + kPairB) * NC + cg]; }
-        }
+        const double wq = (NSP == 1) ? wt[(SQ & 127u) * NC + cg] * wt[(128u + (SQ >> 7)) * NC + cg] : 1.0;
         const double* zup = rb + d.off_z + (cg * NSP) * 4;
         const double* zdn = rb + d.off_z + (cg * NSP + NSP - 1) * 4;
         double val[8];
