@@ -125,7 +125,7 @@ int do_eval(cos_ctx* c, int n, long long batch, const double* gup, const double*
             c->team_tabs[n] = buf;
         }
         a.tabs = c->team_tabs[n];
-    } else if (n >= kPairGlobalMinN) {   // item descriptors of the global-record pair kernel, built on first use
+    } else if (n >= kPairGlobalMinN - 1) {   // item descriptors of the global-record pair kernel, built on first use
         if (!c->team_tabs[n]) {
             const size_t bytes = ((size_t)1 << (n - kPairB)) * kPairDscWords * sizeof(uint32_t);
             unsigned char* buf = nullptr;

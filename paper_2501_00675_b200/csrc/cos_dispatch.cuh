@@ -108,14 +108,22 @@ inline bool has_fused_kernel(int, int, int) { return false; }
 
 // ---- pair kernel on global records (orders 14..16, one species): Z / frontier / reduction arrays in L2 scratch ----
 constexpr int kPairGlobalMinN = 14, kPairGlobalThreads = 512;
-inline bool uses_pair_global(int n, int nsp) { return n >= kPairGlobalMinN && n <= kMaxN && nsp == 1; }
-inline PairChoice pair_global_choice(int n)
+// one species: C = 1 from order 14; two species (G_up != G_down): C = 2 (the two instances of one configuration)
+// from order 13, where the shared-memory variant has room for one instance only
+inline bool uses_pair_global(int n, int nsp)
 {
+    return n <= kMaxN && (nsp == 1 ? n >= kPairGlobalMinN : n >= kPairGlobalMinN - 1);
+}
+inline PairChoice pair_global_choice(int n, int nsp = 1)
+{
+    if (nsp == 2) return {eval_pair_kernel<2, kPairGlobalThreads, 1, 8, true>, pair_dims_global<2>(n, kPairGlobalThreads, 2)};
     return {eval_pair_kernel<1, kPairGlobalThreads, 1, 8, true>, pair_dims_global<1>(n, kPairGlobalThreads)};
 }
 inline size_t pair_global_rec_doubles(int n)
 {
-    return (n >= kPairGlobalMinN && n <= kMaxN) ? (size_t)pair_global_choice(n).d.rec_doubles : 0;
+    if (n < kPairGlobalMinN - 1 || n > kMaxN) return 0;
+    const size_t a = (size_t)pair_global_choice(n, 1).d.rec_doubles, b = (size_t)pair_global_choice(n, 2).d.rec_doubles;
+    return a > b ? a : b;
 }
 
 using TiledKernel = void (*)(EvalArgs, TiledDims);
@@ -135,7 +143,9 @@ inline cudaError_t configure_kernels(int smem_optin)
         e = cudaFuncSetAttribute(pair_choice(n, 1).fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
         if (e != cudaSuccess) return e;
     }
-    e = cudaFuncSetAttribute(pair_global_choice(kPairGlobalMinN).fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
+    e = cudaFuncSetAttribute(pair_global_choice(kPairGlobalMinN, 1).fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
+    if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(pair_global_choice(kPairGlobalMinN, 2).fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
     if (e != cudaSuccess) return e;
     e = cudaFuncSetAttribute(big_kernel(), cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
     if (e != cudaSuccess) return e;
@@ -180,7 +190,7 @@ inline cudaError_t dispatch_eval(const EvalArgs& a, cudaStream_t stream, int num
     }
     if (a.fused) return cudaErrorInvalidValue;   // only the team and pair kernels assemble G on the fly
     if (uses_pair_global(a.n, nsp) && a.scratch != nullptr) {
-        const PairChoice tc = pair_global_choice(a.n);
+        const PairChoice tc = pair_global_choice(a.n, nsp);
         if (tc.d.smem_bytes <= (size_t)smem_optin && (size_t)tc.d.rec_doubles <= a.scratch_stride) {
             int per_sm = 1;
             cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, tc.fn, tc.d.threads, tc.d.smem_bytes);
@@ -189,7 +199,7 @@ inline cudaError_t dispatch_eval(const EvalArgs& a, cudaStream_t stream, int num
             long long grid = (long long)num_sms * per_sm;
             const long long cap = eval_max_ctas(a.n, a.batch, num_sms, smem_optin);
             if (grid > cap) grid = cap;
-            if (grid > a.batch) grid = a.batch;
+            if (grid > a.batch) grid = a.batch;            // one configuration (C / nsp) per team
             tc.fn<<<(unsigned)grid, tc.d.threads, tc.d.smem_bytes, stream>>>(a, tc.d);
             *name = "eval_pair_kernel(global)";
             return cudaGetLastError();

@@ -113,9 +113,9 @@ inline PairDims pair_dims(int n, int nsp, int max_threads = 1024)
 // where it fits); W, the couplings, the tables and the staging buffer stay in shared memory.  Offsets are the same
 // in both spaces (the W part of the scratch block is simply unused).
 template <int C>
-inline PairDims pair_dims_global(int n, int threads)
+inline PairDims pair_dims_global(int n, int threads, int nsp = 1)
 {
-    PairDims d = pair_dims<C>(n, 1);
+    PairDims d = pair_dims<C>(n, nsp);
     d.threads = threads;
     d.pslots = threads / (2 * C);
     d.off_stage = d.off_z;                                // shared memory: W, -u, then the staging buffer
