@@ -100,7 +100,8 @@ int cos_eval_connected_xt(cos_ctx* ctx, int n, long long batch, const int* d_xy,
 
 /* The same whole-path call with HOST buffers (pinned memory recommended): copies h_xy, h_tau (and h_u if
  * not NULL) to the device, runs a1..a5, copies the batch results back into h_out and synchronises
- * the stream before returning.  Used for end-to-end timing (h2d = batch*(8n + 8n [+ 8n]) bytes,
+ * the stream before returning.  Batches of 8192 configurations or more are processed as two halves, the
+ * host-to-device copy of the second half running on an internal copy stream behind the kernels of the first.  Used for end-to-end timing (h2d = batch*(8n + 8n [+ 8n]) bytes,
  * d2h = 8*batch bytes). */
 int cos_eval_connected_xt_host(cos_ctx* ctx, int n, long long batch, const int* h_xy,
                                const double* h_tau, double g_diag, const double* h_u, double U,

@@ -29,6 +29,8 @@ struct cos_ctx {
     unsigned char* team_tabs[COS_MAX_ORDER + 1] = {};            // per order: table image of the team kernel / item
                                                                  // descriptors of the pair kernel
     void* stage = nullptr;          size_t stage_bytes = 0;      // device staging of the host path
+    cudaStream_t copy_stream = nullptr;                          // host path: H2D of chunk k+1 behind the kernels of chunk k
+    cudaEvent_t copy_done[2] = {nullptr, nullptr};
     // bookkeeping
     int last_launches = 0;
     const char* last_kernel = "none";
@@ -242,6 +244,8 @@ int cos_destroy(cos_ctx* c)
     cudaFree(c->gscratch);
     cudaFree(c->stage);
     for (int i = 0; i <= COS_MAX_ORDER; ++i) cudaFree(c->team_tabs[i]);
+    if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
+    for (cudaEvent_t e : c->copy_done) if (e) cudaEventDestroy(e);
     delete c;
     return COS_OK;
 }
@@ -342,13 +346,32 @@ int cos_eval_connected_xt_host(cos_ctx* c, int n, long long batch, const int* h_
     double* d_u = h_u ? (double*)(base + b_tau) : nullptr;
     double* d_out = (double*)(base + b_tau + b_u);
     int* d_xy = (int*)(base + b_tau + b_u + b_out);
-    COS_CUDA(c, cudaMemcpyAsync(d_xy, h_xy, b_xy, cudaMemcpyHostToDevice, c->stream));
-    COS_CUDA(c, cudaMemcpyAsync(d_tau, h_tau, b_tau, cudaMemcpyHostToDevice, c->stream));
-    if (h_u) COS_CUDA(c, cudaMemcpyAsync(d_u, h_u, b_u, cudaMemcpyHostToDevice, c->stream));
-    const int saved = c->last_launches;
-    rc = cos_eval_connected_xt(c, n, batch, d_xy, d_tau, g_diag, d_u, U, d_out);
-    (void)saved;
-    if (rc != COS_OK) return rc;
+    // Two chunks when the batch is large: the host-to-device copy of the second half runs on a copy stream behind
+    // the kernels of the first half.
+    const int nchunk = batch >= 8192 ? 2 : 1;
+    if (nchunk == 2 && !c->copy_stream) {
+        COS_CUDA(c, cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking));
+        for (cudaEvent_t& e : c->copy_done) COS_CUDA(c, cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+    }
+    const long long b0 = nchunk == 2 ? batch / 2 : batch;
+    int launches = 0;
+    for (int k = 0; k < nchunk; ++k) {
+        const long long lo = k == 0 ? 0 : b0, cnt = k == 0 ? b0 : batch - b0;
+        cudaStream_t cs = nchunk == 2 ? c->copy_stream : c->stream;
+        COS_CUDA(c, cudaMemcpyAsync(d_xy + lo * n * 2, h_xy + lo * n * 2, (size_t)cnt * n * 2 * sizeof(int), cudaMemcpyHostToDevice, cs));
+        COS_CUDA(c, cudaMemcpyAsync(d_tau + lo * n, h_tau + lo * n, (size_t)cnt * n * sizeof(double), cudaMemcpyHostToDevice, cs));
+        if (h_u) COS_CUDA(c, cudaMemcpyAsync(d_u + lo * n, h_u + lo * n, (size_t)cnt * n * sizeof(double), cudaMemcpyHostToDevice, cs));
+        if (nchunk == 2) COS_CUDA(c, cudaEventRecord(c->copy_done[k], cs));
+    }
+    for (int k = 0; k < nchunk; ++k) {
+        const long long lo = k == 0 ? 0 : b0, cnt = k == 0 ? b0 : batch - b0;
+        if (nchunk == 2) COS_CUDA(c, cudaStreamWaitEvent(c->stream, c->copy_done[k], 0));
+        rc = cos_eval_connected_xt(c, n, cnt, d_xy + lo * n * 2, d_tau + lo * n, g_diag, d_u ? d_u + lo * n : nullptr, U,
+                                   d_out + lo);
+        if (rc != COS_OK) return rc;
+        launches += c->last_launches;
+    }
+    c->last_launches = launches;
     COS_CUDA(c, cudaMemcpyAsync(h_out, d_out, b_out, cudaMemcpyDeviceToHost, c->stream));
     COS_CUDA(c, cudaStreamSynchronize(c->stream));
     return COS_OK;
