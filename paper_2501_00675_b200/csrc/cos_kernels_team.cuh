@@ -542,6 +542,10 @@ __device__ __forceinline__ void team_reduce(double* CB, double* DB, int ncfg, in
     for (int l = 1; l <= hb; ++l) {
         const int outputs = kBinom.c[hb][l];
         int s = l < R::SMAX ? l : R::SMAX;
+        if (l == hb) {                     // top row: a plain butterfly sums one value, so a whole warp may share it
+            constexpr int SFULL = NC >= 32 ? 0 : (NC == 16 ? 1 : (NC == 8 ? 2 : (NC == 4 ? 3 : (NC == 2 ? 4 : 5))));
+            s = l < SFULL ? l : SFULL;
+        }
         while (s > 0 && (outputs << s) > slots) --s;
         const int per_pass = slots >> s;
         const unsigned c = (unsigned)slot & ((1u << s) - 1u);
