@@ -457,7 +457,7 @@ template <int NC> struct RedLayout {
     static constexpr int ROW = 16 * NC;
     static constexpr int PSTR = 2 * NC;
     static constexpr int MASK = (NC >= 8) ? 0 : (8 / NC - 1);
-    static constexpr int SMAX = (NC >= 32) ? 0 : (NC == 16 ? 1 : (NC == 8 ? 2 : (NC == 4 ? 3 : 4)));
+    static constexpr int SMAX = (NC >= 32) ? 0 : (NC == 16 ? 1 : (NC == 8 ? 2 : (NC == 4 ? 3 : (NC == 2 ? 4 : 5))));
 };
 
 template <int NC>
@@ -657,8 +657,9 @@ __device__ __forceinline__ void team_reduce(double* CB, double* DB, int ncfg, in
                             const bool b3 = (c >> 3) & 1u;
                             const double keep = sel(b3, r2[1], r2[0]);
                             const double send = sel(b3, r2[0], r2[1]);
-                            const double r1 = keep + __shfl_xor_sync(0xffffffffu, send, (NC * 8) & 31);
-                            if (active) { const int e = red_elem<NC>(S, c & 15u, cg); blk[e] = blk[e] - r1; }
+                            double r1 = keep + __shfl_xor_sync(0xffffffffu, send, (NC * 8) & 31);
+                            if (s == 5) r1 += __shfl_xor_sync(0xffffffffu, r1, (NC * 16) & 31);   // NC == 1 only
+                            if (active && !(c & 16u)) { const int e = red_elem<NC>(S, c & 15u, cg); blk[e] = blk[e] - r1; }
                         }
                     }
                 }
