@@ -15,6 +15,8 @@ def torch_mod():
     import torch
     if not torch.cuda.is_available():
         pytest.fail("GPU test selected but no CUDA device: the CUDA path has no CPU fallback")
+    from paper_2501_00675_b200 import build
+    build.build()          # compiles the in-tree library only when it is missing or older than its sources
     return torch
 
 
