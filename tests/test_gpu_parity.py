@@ -102,6 +102,36 @@ def test_eval_every_order_dense(torch_mod, ctx, oracle_mod, n):
         check_parity(oracle_mod, got, Gup, None, 1.7, None, which)
 
 
+# Batches large enough that every persistent CTA loops over at least three teams (or three grid strides of the
+# generic kernel): this drives the prefetch of the next team's matrices, the re-use of the shared-memory / scratch
+# areas between teams and the ragged last team, for EVERY order, one and two species.
+_MANY = {1: 4741, 2: 4741, 3: 4741, 4: 4741, 5: 28417, 6: 28417, 7: 28417, 8: 14209, 9: 7105, 10: 3553,
+         11: 1777, 12: 889, 13: 450, 14: 450, 15: 450, 16: 450}
+
+
+@pytest.mark.parametrize("nsp", [1, 2])
+@pytest.mark.parametrize("n", list(range(1, 17)))
+def test_eval_many_teams_per_cta(torch_mod, ctx, oracle_mod, n, nsp):
+    rng = np.random.default_rng(5000 + 17 * n + nsp)
+    B = _MANY[n]
+    Gup = rng.normal(size=(B, n, n)) / np.sqrt(n) + 0.5 * np.eye(n)
+    Gdn = rng.normal(size=(B, n, n)) / np.sqrt(n) + 0.5 * np.eye(n) if nsp == 2 else None
+    u = rng.uniform(0.5, 2.0, size=(B, n)) if nsp == 2 else None
+    U = 1.0 if nsp == 2 else 1.7
+    # the oracle checks every output up to order 12 and a seeded sample (first and last included) above
+    if n <= 12:
+        idx = np.arange(B)
+    else:
+        idx = np.sort(rng.choice(B, size=8, replace=False))
+        idx[0], idx[-1] = 0, B - 1
+    sub = lambda a: None if a is None else np.ascontiguousarray(a[idx])
+    for which in ("connected", "all"):
+        got = _gpu_eval(torch_mod, ctx, Gup, Gdn, U, u, which)
+        assert np.all(np.isfinite(got))
+        st = check_parity(oracle_mod, got[idx], sub(Gup), sub(Gdn), U, sub(u), which)
+        assert st["exceptions"] == 0, f"well-conditioned dense inputs must meet the strict bar: {st}"
+
+
 @pytest.mark.parametrize("cfg,batch", [(1, 64), (2, 4096), (3, 1024), (4, 256), (5, 16)])
 def test_eval_baseline_configs(torch_mod, ctx, oracle_mod, cfg, batch):
     """BASELINE.json configs (sizes the oracle finishes in seconds), element by element."""
