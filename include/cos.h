@@ -107,6 +107,12 @@ int cos_eval_connected_xt_host(cos_ctx* ctx, int n, long long batch, const int* 
                                const double* h_tau, double g_diag, const double* h_u, double U,
                                double* h_out);
 
+/* Cross-check switch: enable != 0 routes every later cos_eval_* call of this ctx, whatever the order, through the
+ * plain one-thread-per-node kernel (the one orders 1..4 always use) instead of the tuned team / pair kernels; it
+ * runs on the same device with the same arguments and is only slower.  The GPU tests use it to compare the tuned
+ * kernels with a second, structurally different CUDA evaluation of SURVEY.md 8(a) a2..a5. */
+int cos_debug_force_generic(cos_ctx* ctx, int enable);
+
 /* Number of kernel launches issued by the most recent compute call on this ctx (>= 1 on success). */
 int cos_last_launch_count(const cos_ctx* ctx);
 

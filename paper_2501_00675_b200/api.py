@@ -37,6 +37,7 @@ SIGNATURES = {
     "cos_eval_connected": (_int, [_vp, _int, _ll, _vp, _vp, _vp, _dbl, _vp]),
     "cos_eval_connected_xt": (_int, [_vp, _int, _ll, _vp, _vp, _dbl, _vp, _dbl, _vp]),
     "cos_eval_connected_xt_host": (_int, [_vp, _int, _ll, _vp, _vp, _dbl, _vp, _dbl, _vp]),
+    "cos_debug_force_generic": (_int, [_vp, _int]),
     "cos_last_launch_count": (_int, [_vp]),
     "cos_last_kernel_name": (ctypes.c_char_p, [_vp]),
     "cos_enable_kernel_timer": (_int, [_vp, _int]),
@@ -95,8 +96,18 @@ def _ptr(t):
     return ctypes.c_void_p(t.ctypes.data)
 
 
+def _kind(t):
+    """('f64' | 'i32' | other, shape tuple) of a torch tensor or numpy array."""
+    name = str(t.dtype).replace("torch.", "")
+    return {"float64": "f64", "int32": "i32"}.get(name, name), tuple(int(x) for x in t.shape)
+
+
 class Context:
-    """Owner of one cos_ctx.  All tensors passed to the d_* arguments must live on `device`."""
+    """Owner of one cos_ctx.  All tensors passed to the d_* arguments must live on `device`.
+
+    The ctx launches on the stream given at construction (default: torch's current stream of the device at that
+    moment); work the caller enqueues on another stream must be ordered with it by the caller.  Every call leaves
+    `device` as the current CUDA device of the calling thread."""
 
     def __init__(self, device: int | None = None, stream=None):
         import torch  # device memory and streams only
@@ -141,39 +152,85 @@ class Context:
                 text += ": " + self._lib.cos_last_cuda_error(self._h).decode()
             raise CosError(rc, text)
 
+    def _dev(self, t, kind, shape, name, optional=False):
+        """Marshalling guard: dtype, shape, contiguity and residency of a d_* argument (no arithmetic)."""
+        if t is None:
+            if optional:
+                return None
+            raise CosError(COS_EINVAL, f"{name} is required")
+        k, shp = _kind(t)
+        if k != kind:
+            raise CosError(COS_EINVAL, f"{name}: dtype {t.dtype}, expected {'float64' if kind == 'f64' else 'int32'}")
+        if shape is not None and shp != tuple(shape):
+            raise CosError(COS_EINVAL, f"{name}: shape {shp}, expected {tuple(shape)}")
+        if not getattr(t, "is_cuda", False) or t.device.index != self.device:
+            raise CosError(COS_EINVAL, f"{name}: must be a CUDA tensor on device {self.device}")
+        if not t.is_contiguous():
+            raise CosError(COS_EINVAL, f"{name}: must be contiguous")
+        return _ptr(t)
+
+    @staticmethod
+    def _host(t, kind, shape, name, optional=False):
+        if t is None:
+            if optional:
+                return None
+            raise CosError(COS_EINVAL, f"{name} is required")
+        k, shp = _kind(t)
+        if k != kind or shp != tuple(shape):
+            raise CosError(COS_EINVAL, f"{name}: {t.dtype} {shp}, expected {kind} {tuple(shape)}")
+        if getattr(t, "is_cuda", False):
+            raise CosError(COS_EINVAL, f"{name}: must be a host buffer")
+        contiguous = t.is_contiguous() if hasattr(t, "is_contiguous") else t.flags["C_CONTIGUOUS"]
+        if not contiguous:
+            raise CosError(COS_EINVAL, f"{name}: must be contiguous")
+        return _ptr(t)
+
     # -- the boundary ---------------------------------------------------------------------
     def set_g0_table(self, d_table, beta: float, spin: int = -1):
         """d_table: CUDA float64 tensor [Lx, Ly, ntau] (tau fastest); kept alive by this object."""
         Lx, Ly, ntau = (int(s) for s in d_table.shape)
-        assert d_table.is_cuda and d_table.is_contiguous() and d_table.dtype.itemsize == 8
-        self._check(self._lib.cos_set_g0_table(self._h, int(spin), _ptr(d_table), Lx, Ly, ntau, float(beta)))
+        p = self._dev(d_table, "f64", (Lx, Ly, ntau), "d_table")
+        self._check(self._lib.cos_set_g0_table(self._h, int(spin), p, Lx, Ly, ntau, float(beta)))
         self._table_refs[spin] = d_table
 
     def build_G(self, d_xy, d_tau, d_Gup, d_Gdn=None, g_diag: float = 0.0):
         batch, n = (int(s) for s in d_tau.shape)
-        self._check(self._lib.cos_build_G(self._h, n, batch, _ptr(d_xy), _ptr(d_tau), float(g_diag),
-                                          _ptr(d_Gup), _ptr(d_Gdn)))
+        self._check(self._lib.cos_build_G(self._h, n, batch, self._dev(d_xy, "i32", (batch, n, 2), "d_xy"),
+                                          self._dev(d_tau, "f64", (batch, n), "d_tau"), float(g_diag),
+                                          self._dev(d_Gup, "f64", (batch, n, n), "d_Gup"),
+                                          self._dev(d_Gdn, "f64", (batch, n, n), "d_Gdn", optional=True)))
+
+    def _eval_ptrs(self, d_Gup, d_Gdn, d_out, d_u):
+        batch, n = int(d_Gup.shape[0]), int(d_Gup.shape[1])
+        return (n, batch, self._dev(d_Gup, "f64", (batch, n, n), "d_Gup"), self._dev(d_Gdn, "f64", (batch, n, n), "d_Gdn"),
+                self._dev(d_u, "f64", (batch, n), "d_u", optional=True), self._dev(d_out, "f64", (batch,), "d_out"))
 
     def eval_all(self, d_Gup, d_Gdn, d_out, U: float = 1.0, d_u=None):
-        batch, n = int(d_Gup.shape[0]), int(d_Gup.shape[1])
-        self._check(self._lib.cos_eval_all(self._h, n, batch, _ptr(d_Gup), _ptr(d_Gdn), _ptr(d_u),
-                                           float(U), _ptr(d_out)))
+        n, batch, gu, gd, u, out = self._eval_ptrs(d_Gup, d_Gdn, d_out, d_u)
+        self._check(self._lib.cos_eval_all(self._h, n, batch, gu, gd, u, float(U), out))
 
     def eval_connected(self, d_Gup, d_Gdn, d_out, U: float = 1.0, d_u=None):
-        batch, n = int(d_Gup.shape[0]), int(d_Gup.shape[1])
-        self._check(self._lib.cos_eval_connected(self._h, n, batch, _ptr(d_Gup), _ptr(d_Gdn), _ptr(d_u),
-                                                 float(U), _ptr(d_out)))
+        n, batch, gu, gd, u, out = self._eval_ptrs(d_Gup, d_Gdn, d_out, d_u)
+        self._check(self._lib.cos_eval_connected(self._h, n, batch, gu, gd, u, float(U), out))
 
     def eval_connected_xt(self, d_xy, d_tau, d_out, U: float = 1.0, d_u=None, g_diag: float = 0.0):
         batch, n = (int(s) for s in d_tau.shape)
-        self._check(self._lib.cos_eval_connected_xt(self._h, n, batch, _ptr(d_xy), _ptr(d_tau),
-                                                    float(g_diag), _ptr(d_u), float(U), _ptr(d_out)))
+        self._check(self._lib.cos_eval_connected_xt(
+            self._h, n, batch, self._dev(d_xy, "i32", (batch, n, 2), "d_xy"), self._dev(d_tau, "f64", (batch, n), "d_tau"),
+            float(g_diag), self._dev(d_u, "f64", (batch, n), "d_u", optional=True), float(U),
+            self._dev(d_out, "f64", (batch,), "d_out")))
 
     def eval_connected_xt_host(self, h_xy, h_tau, h_out, U: float = 1.0, h_u=None, g_diag: float = 0.0):
         """Host buffers (numpy arrays or pinned CPU tensors); synchronises before returning."""
         batch, n = (int(s) for s in h_tau.shape)
-        self._check(self._lib.cos_eval_connected_xt_host(self._h, n, batch, _ptr(h_xy), _ptr(h_tau),
-                                                         float(g_diag), _ptr(h_u), float(U), _ptr(h_out)))
+        self._check(self._lib.cos_eval_connected_xt_host(
+            self._h, n, batch, self._host(h_xy, "i32", (batch, n, 2), "h_xy"), self._host(h_tau, "f64", (batch, n), "h_tau"),
+            float(g_diag), self._host(h_u, "f64", (batch, n), "h_u", optional=True), float(U),
+            self._host(h_out, "f64", (batch,), "h_out")))
+
+    def force_generic(self, on: bool = True):
+        """Cross-check switch (include/cos.h: cos_debug_force_generic)."""
+        self._check(self._lib.cos_debug_force_generic(self._h, 1 if on else 0))
 
     # -- bookkeeping and probes -------------------------------------------------------------
     def last_launch_count(self) -> int:

@@ -8,6 +8,7 @@
 #include <vector>
 
 #include "cos_common.cuh"
+#include "cos_internal.h"
 #include "cos_kernels_generic.cuh"
 #include "cos_dispatch.cuh"
 
@@ -32,6 +33,7 @@ struct cos_ctx {
     cudaStream_t copy_stream = nullptr;                          // host path: H2D of chunk k+1 behind the kernels of chunk k
     cudaEvent_t copy_done[2] = {nullptr, nullptr};
     // bookkeeping
+    bool force_generic = false;     // cos_debug_force_generic: every order through eval_generic_kernel
     int last_launches = 0;
     const char* last_kernel = "none";
     cudaError_t last_err = cudaSuccess;
@@ -70,6 +72,13 @@ int grow(cos_ctx* c, void** p, size_t* have, size_t need)
     return COS_OK;
 }
 
+int alloc_dev(cos_ctx* c, void** p, size_t bytes)
+{
+    cudaError_t e = cudaMalloc(p, bytes);
+    if (e != cudaSuccess) { c->last_err = e; (void)cudaGetLastError(); *p = nullptr; return COS_ENOMEM; }
+    return COS_OK;
+}
+
 bool timer_begin(cos_ctx* c)
 {
     if (!c->timing) return false;
@@ -102,7 +111,7 @@ int launch_eval(cos_ctx* c, const EvalArgs& args)
     const bool t = timer_begin(c);
     int launches = 0;
     const char* name = nullptr;
-    cudaError_t e = dispatch_eval(args, c->stream, c->num_sms, c->smem_optin, &launches, &name);
+    cudaError_t e = dispatch_eval(args, c->stream, c->num_sms, c->smem_optin, c->force_generic, &launches, &name);
     if (t) timer_end(c);
     if (e != cudaSuccess) return fail_cuda(c, e);
     c->last_launches += launches;
@@ -117,11 +126,13 @@ int do_eval(cos_ctx* c, int n, long long batch, const double* gup, const double*
     EvalArgs a{};
     a.n = n; a.batch = batch; a.Gup = gup; a.Gdn = gdn; a.u = u; a.U = U; a.out = out;
     a.connected = connected; a.off = c->off;
-    if (uses_team(n)) {          // table image of this order, built on first use
+    if (c->force_generic) {
+        // no tables: the generic kernel computes its indices on the fly
+    } else if (uses_team(n)) {   // table image of this order, built on first use
         if (!c->team_tabs[n]) {
             const TeamDims td = team_choice(n, 1).d;
             unsigned char* buf = nullptr;
-            if (cudaMalloc((void**)&buf, (size_t)td.tab_bytes) != cudaSuccess) return COS_ENOMEM;
+            if (alloc_dev(c, (void**)&buf, (size_t)td.tab_bytes) != COS_OK) return COS_ENOMEM;
             team_tables_kernel<<<1, 256, (size_t)td.tab_bytes, c->stream>>>(td, buf);
             COS_CUDA(c, cudaGetLastError());
             c->team_tabs[n] = buf;
@@ -131,7 +142,7 @@ int do_eval(cos_ctx* c, int n, long long batch, const double* gup, const double*
         if (!c->team_tabs[n]) {
             const size_t bytes = ((size_t)1 << (n - kPairB)) * kPairDscWords * sizeof(uint32_t);
             unsigned char* buf = nullptr;
-            if (cudaMalloc((void**)&buf, bytes) != cudaSuccess) return COS_ENOMEM;
+            if (alloc_dev(c, (void**)&buf, bytes) != COS_OK) return COS_ENOMEM;
             pair_tables_kernel<<<32, 256, 0, c->stream>>>(n, reinterpret_cast<uint32_t*>(buf));
             COS_CUDA(c, cudaGetLastError());
             c->team_tabs[n] = buf;
@@ -139,9 +150,9 @@ int do_eval(cos_ctx* c, int n, long long batch, const double* gup, const double*
         a.tabs = c->team_tabs[n];
     }
     // global scratch for the orders whose frontier does not fit in shared memory
-    const size_t per_cta = eval_scratch_doubles(n, c->smem_optin);
+    const size_t per_cta = eval_scratch_doubles(n, c->smem_optin, c->force_generic);
     if (per_cta) {
-        const int ctas = eval_max_ctas(n, batch, c->num_sms, c->smem_optin);
+        const int ctas = eval_max_ctas(batch, c->num_sms);
         int rc = grow(c, (void**)&c->scratch, &c->scratch_bytes, per_cta * sizeof(double) * (size_t)ctas);
         if (rc != COS_OK) return rc;
         a.scratch = c->scratch;
@@ -305,16 +316,6 @@ int cos_eval_connected_xt(cos_ctx* c, int n, long long batch, const int* d_xy, c
     c->last_launches = 0;
     if (batch == 0) return COS_OK;
     const bool two = c->table[1] && c->table[1] != c->table[0];
-    if (has_fused_kernel(n, two ? 2 : 1, c->smem_optin)) {
-        // a1 fused into the evaluation kernel: G is assembled straight into shared memory
-        EvalArgs a{};
-        a.n = n; a.batch = batch; a.u = d_u; a.U = U; a.out = d_out; a.connected = 1; a.off = c->off;
-        a.fused = 1;
-        a.bg.n = n; a.bg.batch = batch; a.bg.xy = d_xy; a.bg.tau = d_tau;
-        a.bg.Tup = c->table[0]; a.bg.Tdn = two ? c->table[1] : c->table[0];
-        a.bg.Lx = c->Lx; a.bg.Ly = c->Ly; a.bg.ntau = c->ntau; a.bg.beta = c->beta; a.bg.g_diag = g_diag;
-        return launch_eval(c, a);
-    }
     const size_t one = (size_t)batch * n * n * sizeof(double);
     int rc = grow(c, (void**)&c->gscratch, &c->gscratch_bytes, two ? 2 * one : one);
     if (rc != COS_OK) return rc;
@@ -377,6 +378,16 @@ int cos_eval_connected_xt_host(cos_ctx* c, int n, long long batch, const int* h_
     return COS_OK;
 }
 
+int cos_internal_device(const cos_ctx* c) { return c->device; }
+void* cos_internal_stream(const cos_ctx* c) { return (void*)c->stream; }
+
+int cos_debug_force_generic(cos_ctx* c, int enable)
+{
+    if (!c) return COS_EINVAL;
+    c->force_generic = enable != 0;
+    return COS_OK;
+}
+
 int cos_last_launch_count(const cos_ctx* c) { return c ? c->last_launches : 0; }
 const char* cos_last_kernel_name(const cos_ctx* c) { return c ? c->last_kernel : "none"; }
 
@@ -429,17 +440,3 @@ long long cos_flop_count(int n, int n_species, int connected)
 }
 
 }  // extern "C"
-
-#ifdef COS_PHASE_TIMING
-// Development aid (not part of include/cos.h; compiled only with -DCOS_PHASE_TIMING): cycles thread 0 of every
-// CTA spent in each phase of the evaluation kernels, summed over CTAs.
-extern "C" int cos_debug_phase_cycles(unsigned long long* h_out32, int reset)
-{
-    if (h_out32 && cudaMemcpyFromSymbol(h_out32, cosb::g_phase_cycles, 32 * sizeof(unsigned long long)) != cudaSuccess) return COS_ECUDA;
-    if (reset) {
-        unsigned long long z[32] = {0};
-        if (cudaMemcpyToSymbol(cosb::g_phase_cycles, z, sizeof(z)) != cudaSuccess) return COS_ECUDA;
-    }
-    return COS_OK;
-}
-#endif

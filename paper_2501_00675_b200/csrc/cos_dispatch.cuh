@@ -1,18 +1,20 @@
 // cos_dispatch.cuh -- picks the kernel variant for an evaluation launch and sizes its resources.
+//   n = 1..4                        eval_generic_kernel   (one thread per node, frontier in shared memory)
+//   n = 5..10                       eval_team_kernel      (C instances per CTA, thread-bit register tiles)
+//   n = 11..13 (one species <= 13,
+//               two species <= 12)  eval_pair_kernel      (items split over lane pairs, shared memory)
+//   n = 14..16, two species n = 13  eval_pair_kernel<..., GLOBAL = true>  (records in per-CTA global scratch)
+// The generic kernel also runs any order when the context is told to (cos_debug_force_generic): it is the
+// in-library cross-check of the tuned kernels, not a fallback for another device.
 #pragma once
 #include "cos_common.cuh"
 #include "cos_kernels_generic.cuh"
-#include "cos_kernels_tiled.cuh"
 #include "cos_kernels_team.cuh"
 #include "cos_kernels_pair.cuh"
 
 namespace cosb {
 
 constexpr int kGenericThreads = 256;
-constexpr int kTiledB = 3;
-constexpr int kTiledThreads = 128;
-constexpr int kTiledNA = 4, kTiledJB = 5;
-constexpr int kTiledMinN = 5, kTiledMaxN = 12;
 
 inline size_t generic_smem_bytes(int n, int nsp)
 {
@@ -25,53 +27,9 @@ inline bool generic_needs_global(int n, int smem_optin)
     return generic_smem_bytes(n, 2) > (size_t)smem_optin;
 }
 
-// Configurations per CTA of the tiled kernel (0: the tiled kernel cannot run this order).
-inline int tiled_group(int n, int nsp, int smem_optin)
+inline size_t generic_scratch_doubles(int n, int smem_optin)
 {
-    if (n < kTiledMinN || n > kTiledMaxN) return 0;
-    if (tiled_smem_bytes<kTiledB>(n, 1, nsp) > (size_t)smem_optin) return 0;
-    const int q = n - kTiledB - 1;                       // widest stage
-    const int widest = kBinomHost.c[q][q / 2];
-    int G = (kTiledThreads + widest - 1) / widest;
-    const size_t budget = 112 * 1024;                    // keep two CTAs per SM where possible
-    while (G > 1 && tiled_smem_bytes<kTiledB>(n, G, nsp) > budget) --G;
-    return G;
-}
-
-inline bool uses_tiled(int n, int nsp, int smem_optin) { return tiled_group(n, nsp, smem_optin) > 0; }
-
-// Orders 13..16: the tiled kernel with one configuration per CTA whose block (W, Z, level buffers, reduction
-// arrays) lives in global scratch (L2 resident); only the subset tables stay in shared memory.
-constexpr int kBigThreads = 256, kBigNA = 6, kBigJB = 7, kBigMinN = 13;
-inline bool uses_big(int n) { return n >= kBigMinN && n <= kMaxN; }
-inline TiledDims big_dims(int n, int nsp)
-{
-    TiledDims d = tiled_dims<kTiledB>(n, 1, nsp);
-    d.use_global = 1;
-    return d;
-}
-
-inline size_t pair_global_rec_doubles(int n);   // defined with the pair-kernel choices below
-
-// Doubles of global scratch per CTA (0: everything lives in shared memory).
-inline size_t eval_scratch_doubles(int n, int smem_optin)
-{
-    if (uses_big(n)) {
-        size_t v = (size_t)big_dims(n, 2).cfg_doubles;
-        const size_t p = pair_global_rec_doubles(n);     // the pair kernel on global records (orders 14..16)
-        if (p > v) v = p;
-        return v;
-    }
-    if (uses_tiled(n, 2, smem_optin)) return 0;
-    if (!generic_needs_global(n, smem_optin)) return 0;
-    return ((size_t)2 << n) + generic_frontier_doubles(n);
-}
-
-inline int eval_max_ctas(int n, long long batch, int num_sms, int smem_optin)
-{
-    (void)n; (void)smem_optin;
-    const long long cap = (long long)num_sms * 2;
-    return (int)(batch < cap ? batch : cap);
+    return generic_needs_global(n, smem_optin) ? ((size_t)2 << n) + generic_frontier_doubles(n) : 0;
 }
 
 // ---- team kernel (orders 5..10): instances per team and launch shape per order ----
@@ -87,29 +45,20 @@ inline TeamChoice team_choice(int n, int nsp)
     return {eval_team_kernel<32, 192, 2>, team_dims<32>(n, nsp)};
 }
 
-// ---- pair kernel (orders 11..12): the team mapping with every item split over a lane pair ----
+// ---- pair kernel (orders 11..13): the team mapping with every item split over a lane pair ----
 constexpr int kPairMinN = 11, kPairMaxN = 13;
 using PairKernel = void (*)(EvalArgs, PairDims);
 struct PairChoice { PairKernel fn; PairDims d; };
-inline bool uses_pair(int n) { return n >= kPairMinN && n <= kPairMaxN; }
-// True when order n has a kernel that assembles G on the fly (cos_eval_connected_xt without a G round trip).
-inline bool has_fused_kernel(int n, int nsp, int smem_optin);
+inline bool uses_pair(int n, int nsp) { return n >= kPairMinN && n <= (nsp == 1 ? kPairMaxN : kPairMaxN - 1); }
 inline PairChoice pair_choice(int n, int nsp)
 {
-    if (n == 13) return {eval_pair_kernel<1, 512, 1, 10>, pair_dims<1>(n, 1)};   // one species only (see dispatch_eval)
+    if (n == 13) return {eval_pair_kernel<1, 512, 1, 10>, pair_dims<1>(n, 1)};   // one species only
     if (n == 12) return {eval_pair_kernel<2, 512, 1, 9>, pair_dims<2>(n, nsp)};
     return {eval_pair_kernel<4, 512, 1, 8>, pair_dims<4>(n, nsp, 512)};
 }
 
-// No evaluation kernel assembles G on the fly any more: a separate cos_build_G launch plus a cp.async prefetch of
-// the next team's matrices measured faster than the in-kernel gather (whose two dependent global round trips per
-// team sat on the critical path), and G costs 16 n^2 bytes per configuration of HBM traffic -- noise.
-inline bool has_fused_kernel(int, int, int) { return false; }
-
-// ---- pair kernel on global records (orders 14..16, one species): Z / frontier / reduction arrays in L2 scratch ----
+// ---- pair kernel on global records (orders 14..16; two species from 13): Z / frontier / reduction arrays in L2 scratch ----
 constexpr int kPairGlobalMinN = 14, kPairGlobalThreads = 512;
-// one species: C = 1 from order 14; two species (G_up != G_down): C = 2 (the two instances of one configuration)
-// from order 13, where the shared-memory variant has room for one instance only
 inline bool uses_pair_global(int n, int nsp)
 {
     return n <= kMaxN && (nsp == 1 ? n >= kPairGlobalMinN : n >= kPairGlobalMinN - 1);
@@ -126,9 +75,18 @@ inline size_t pair_global_rec_doubles(int n)
     return a > b ? a : b;
 }
 
-using TiledKernel = void (*)(EvalArgs, TiledDims);
-inline TiledKernel tiled_kernel() { return eval_tiled_kernel<kTiledB, kTiledThreads, kTiledNA, kTiledJB, false>; }
-inline TiledKernel big_kernel() { return eval_tiled_kernel<kTiledB, kBigThreads, kBigNA, kBigJB, true>; }
+// Doubles of global scratch per CTA (0: everything lives in shared memory).
+inline size_t eval_scratch_doubles(int n, int smem_optin, bool force_generic)
+{
+    if (force_generic) return generic_scratch_doubles(n, smem_optin);
+    return pair_global_rec_doubles(n);
+}
+
+inline int eval_max_ctas(long long batch, int num_sms)
+{
+    const long long cap = (long long)num_sms * 2;
+    return (int)(batch < cap ? batch : cap);
+}
 
 inline cudaError_t configure_kernels(int smem_optin)
 {
@@ -145,96 +103,47 @@ inline cudaError_t configure_kernels(int smem_optin)
     }
     e = cudaFuncSetAttribute(pair_global_choice(kPairGlobalMinN, 1).fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
     if (e != cudaSuccess) return e;
-    e = cudaFuncSetAttribute(pair_global_choice(kPairGlobalMinN, 2).fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
+    return cudaFuncSetAttribute(pair_global_choice(kPairGlobalMinN, 2).fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
+}
+
+template <class Kernel, class Dims>
+inline cudaError_t launch_persistent(Kernel fn, const Dims& d, const EvalArgs& a, long long teams, long long cap,
+                                     int num_sms, cudaStream_t stream)
+{
+    int per_sm = 1;
+    cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, d.threads, d.smem_bytes);
     if (e != cudaSuccess) return e;
-    e = cudaFuncSetAttribute(big_kernel(), cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
-    if (e != cudaSuccess) return e;
-    return cudaFuncSetAttribute(tiled_kernel(), cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
+    if (per_sm < 1) per_sm = 1;
+    long long grid = (long long)num_sms * per_sm;
+    if (grid > teams) grid = teams;
+    if (cap > 0 && grid > cap) grid = cap;
+    fn<<<(unsigned)grid, d.threads, d.smem_bytes, stream>>>(a, d);
+    return cudaGetLastError();
 }
 
 inline cudaError_t dispatch_eval(const EvalArgs& a, cudaStream_t stream, int num_sms, int smem_optin,
-                                 int* launches, const char** name)
+                                 bool force_generic, int* launches, const char** name)
 {
-    const int nsp = a.fused ? (a.bg.Tdn != a.bg.Tup ? 2 : 1) : ((a.Gdn == a.Gup) ? 1 : 2);
+    const int nsp = (a.Gdn == a.Gup) ? 1 : 2;
     *launches = 1;
-    if (uses_team(a.n)) {
+    if (!force_generic && uses_team(a.n)) {
         const TeamChoice tc = team_choice(a.n, nsp);
-        if (tc.d.smem_bytes <= (size_t)smem_optin) {
-            int per_sm = 1;
-            const int block = tc.d.threads;
-            cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, tc.fn, block, tc.d.smem_bytes);
-            if (e != cudaSuccess) return e;
-            if (per_sm < 1) per_sm = 1;
-            const long long teams = (a.batch * nsp + tc.d.C - 1) / tc.d.C;
-            long long grid = (long long)num_sms * per_sm;
-            if (grid > teams) grid = teams;
-            tc.fn<<<(unsigned)grid, block, tc.d.smem_bytes, stream>>>(a, tc.d);
-            *name = "eval_team_kernel";
-            return cudaGetLastError();
-        }
+        *name = "eval_team_kernel";
+        return launch_persistent(tc.fn, tc.d, a, (a.batch * nsp + tc.d.C - 1) / tc.d.C, 0, num_sms, stream);
     }
-    if (uses_pair(a.n)) {
+    if (!force_generic && uses_pair(a.n, nsp)) {
         const PairChoice tc = pair_choice(a.n, nsp);
-        if (tc.d.smem_bytes <= (size_t)smem_optin && tc.d.C >= nsp) {
-            int per_sm = 1;
-            cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, tc.fn, tc.d.threads, tc.d.smem_bytes);
-            if (e != cudaSuccess) return e;
-            if (per_sm < 1) per_sm = 1;
-            const long long teams = (a.batch * nsp + tc.d.C - 1) / tc.d.C;
-            long long grid = (long long)num_sms * per_sm;
-            if (grid > teams) grid = teams;
-            tc.fn<<<(unsigned)grid, tc.d.threads, tc.d.smem_bytes, stream>>>(a, tc.d);
-            *name = "eval_pair_kernel";
-            return cudaGetLastError();
-        }
+        *name = "eval_pair_kernel";
+        return launch_persistent(tc.fn, tc.d, a, (a.batch * nsp + tc.d.C - 1) / tc.d.C, 0, num_sms, stream);
     }
-    if (a.fused) return cudaErrorInvalidValue;   // only the team and pair kernels assemble G on the fly
-    if (uses_pair_global(a.n, nsp) && a.scratch != nullptr) {
+    if (!force_generic && uses_pair_global(a.n, nsp)) {
         const PairChoice tc = pair_global_choice(a.n, nsp);
-        if (tc.d.smem_bytes <= (size_t)smem_optin && (size_t)tc.d.rec_doubles <= a.scratch_stride) {
-            int per_sm = 1;
-            cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, tc.fn, tc.d.threads, tc.d.smem_bytes);
-            if (e != cudaSuccess) return e;
-            if (per_sm < 1) per_sm = 1;
-            long long grid = (long long)num_sms * per_sm;
-            const long long cap = eval_max_ctas(a.n, a.batch, num_sms, smem_optin);
-            if (grid > cap) grid = cap;
-            if (grid > a.batch) grid = a.batch;            // one configuration (C / nsp) per team
-            tc.fn<<<(unsigned)grid, tc.d.threads, tc.d.smem_bytes, stream>>>(a, tc.d);
-            *name = "eval_pair_kernel(global)";
-            return cudaGetLastError();
-        }
-    }
-    if (uses_big(a.n)) {
-        const TiledDims d = big_dims(a.n, nsp);
-        const size_t smem = (size_t)d.tab_bytes;
-        int per_sm = 1;
-        cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, big_kernel(), kBigThreads, smem);
-        if (e != cudaSuccess) return e;
-        if (per_sm < 1) per_sm = 1;
-        long long grid = (long long)num_sms * per_sm;
-        const long long cap = eval_max_ctas(a.n, a.batch, num_sms, smem_optin);
-        if (grid > cap) grid = cap;
-        big_kernel()<<<(unsigned)grid, kBigThreads, smem, stream>>>(a, d);
-        *name = "eval_tiled_kernel(global)";
-        return cudaGetLastError();
-    }
-    const int G = tiled_group(a.n, nsp, smem_optin);
-    if (G > 0) {
-        const TiledDims d = tiled_dims<kTiledB>(a.n, G, nsp);
-        const size_t smem = tiled_smem_bytes<kTiledB>(a.n, G, nsp);
-        int per_sm = 1;
-        cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, tiled_kernel(), kTiledThreads, smem);
-        if (e != cudaSuccess) return e;
-        if (per_sm < 1) per_sm = 1;
-        const long long groups = (a.batch + G - 1) / G;
-        long long grid = (long long)num_sms * per_sm;
-        if (grid > groups) grid = groups;
-        tiled_kernel()<<<(unsigned)grid, kTiledThreads, smem, stream>>>(a, d);
-        *name = "eval_tiled_kernel";
-        return cudaGetLastError();
+        if (a.scratch == nullptr || (size_t)tc.d.rec_doubles > a.scratch_stride) return cudaErrorInvalidValue;
+        *name = "eval_pair_kernel(global)";
+        return launch_persistent(tc.fn, tc.d, a, a.batch, eval_max_ctas(a.batch, num_sms), num_sms, stream);
     }
     const bool use_global = generic_needs_global(a.n, smem_optin);
+    if (use_global && a.scratch == nullptr) return cudaErrorInvalidValue;
     const size_t smem = use_global ? sizeof(double) * generic_small_doubles(a.n) : generic_smem_bytes(a.n, nsp);
     int per_sm = 1;
     cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, eval_generic_kernel<kGenericThreads>,
@@ -243,7 +152,7 @@ inline cudaError_t dispatch_eval(const EvalArgs& a, cudaStream_t stream, int num
     if (per_sm < 1) per_sm = 1;
     long long grid = (long long)num_sms * per_sm;
     if (use_global) {
-        const long long cap = eval_max_ctas(a.n, a.batch, num_sms, smem_optin);
+        const long long cap = eval_max_ctas(a.batch, num_sms);
         if (grid > cap) grid = cap;
     }
     if (grid > a.batch) grid = a.batch;

@@ -25,7 +25,6 @@
 #pragma once
 #include "cos_common.cuh"
 #include "cos_kernels_generic.cuh"
-#include "cos_kernels_tiled.cuh"   // kBinom, cpopc
 #include "cos_kernels_team.cuh"    // RedLayout, team_reduce (connected reduction on interleaved blocks)
 
 namespace cosb {

@@ -28,7 +28,6 @@
 #pragma once
 #include "cos_common.cuh"
 #include "cos_kernels_generic.cuh"
-#include "cos_kernels_tiled.cuh"   // kBinom, cpopc
 
 namespace cosb {
 

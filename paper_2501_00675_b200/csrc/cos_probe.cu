@@ -4,6 +4,7 @@
 #include <cuda_runtime.h>
 
 #include "../../include/cos.h"
+#include "cos_internal.h"
 
 namespace {
 
@@ -67,19 +68,20 @@ int time_best_ms(cudaStream_t stream, F launch, float* best)
 
 extern "C" {
 
-// The ctx is opaque here; the probes only need its device to be current, which every compute call
-// of the ctx guarantees.  They run on the legacy default stream and synchronise.
+// The probes run on the device and the stream of the ctx and synchronise that stream.
 int cos_probe_dfma(cos_ctx* ctx, double* tflops)
 {
     if (!ctx || !tflops) return COS_EINVAL;
-    int dev = 0, sms = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess) return COS_ECUDA;
+    const int dev = cos_internal_device(ctx);
+    int sms = 0;
+    if (cudaSetDevice(dev) != cudaSuccess) return COS_ECUDA;
+    cudaStream_t st = (cudaStream_t)cos_internal_stream(ctx);
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     double* d = nullptr;
     if (cudaMalloc((void**)&d, 64) != cudaSuccess) return COS_ENOMEM;
     const int iters = 4096, blocks = sms * 8, threads = 256;
     float best = 0.f;
-    int rc = time_best_ms(nullptr, [&] { dfma_probe_kernel<<<blocks, threads>>>(d, iters, 1.0000001, 1e-9); }, &best);
+    int rc = time_best_ms(st, [&] { dfma_probe_kernel<<<blocks, threads, 0, st>>>(d, iters, 1.0000001, 1e-9); }, &best);
     cudaFree(d);
     if (rc != COS_OK) return rc;
     const double flop = 2.0 * (double)blocks * threads * (double)iters * kChains;
@@ -90,14 +92,16 @@ int cos_probe_dfma(cos_ctx* ctx, double* tflops)
 int cos_probe_smem(cos_ctx* ctx, double* gbytes_per_s)
 {
     if (!ctx || !gbytes_per_s) return COS_EINVAL;
-    int dev = 0, sms = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess) return COS_ECUDA;
+    const int dev = cos_internal_device(ctx);
+    int sms = 0;
+    if (cudaSetDevice(dev) != cudaSuccess) return COS_ECUDA;
+    cudaStream_t st = (cudaStream_t)cos_internal_stream(ctx);
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     double* d = nullptr;
     if (cudaMalloc((void**)&d, 64) != cudaSuccess) return COS_ENOMEM;
     const int iters = 8192, blocks = sms * 2, threads = 1024;
     float best = 0.f;
-    int rc = time_best_ms(nullptr, [&] { smem_probe_kernel<<<blocks, threads>>>(d, iters); }, &best);
+    int rc = time_best_ms(st, [&] { smem_probe_kernel<<<blocks, threads, 0, st>>>(d, iters); }, &best);
     cudaFree(d);
     if (rc != COS_OK) return rc;
     const double bytes = 8.0 * 4.0 * (double)blocks * threads * (double)iters;

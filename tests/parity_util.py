@@ -1,4 +1,4 @@
-"""The parity rule of DESIGN.md §3, in one place.
+"""The parity rule of DESIGN.md §4 ("Tolerance and the exception rule"), in one place.
 
 north_star: "GPU results must match the oracle on the same seeded inputs to a relative error of
 <= 1e-10 in FP64".  `connected` is obtained by subtracting disconnected parts (reading R5), so for a
@@ -11,13 +11,22 @@ are merely relabelled (an exact symmetry of the sum).  The rule therefore is
       oracle run with long-double accumulators and sigma is the RMS deviation from truth of the FP64
       oracle over K = 16 random relabellings of the vertices (i.e. the GPU is no less accurate than
       FP64 arithmetic is for that configuration), and
-  (3) the number of such exceptions is at most max(1, 1 %) of the batch.
+  (3) the number of such exceptions is at most max(1, ceil(f * batch)) with f = 0.2 % by default and f = 1 % for
+      the clustered-time workload cfg4, whose FP64 oracle itself misses the bar against its long-double mode on
+      5 of 1024 configurations (DESIGN.md §4 lists the measured counts).
+
+Every call appends its statistics to STATS; tests/conftest.py prints them in the terminal summary, so the number of
+exceptions each test used is on record even under `pytest -q`.
 """
+import math
+
 import numpy as np
 
 REL_TOL = 1e-10
 K_RELABEL = 16
-MAX_EXCEPTION_FRACTION = 0.01
+MAX_EXCEPTION_FRACTION = 0.002
+CLUSTERED_EXCEPTION_FRACTION = 0.01
+STATS = []          # one dict per check_parity call (label, batch, exceptions, ...)
 
 
 def oracle_reference(oracle_mod, Gup, Gdn, U, u):
@@ -25,7 +34,7 @@ def oracle_reference(oracle_mod, Gup, Gdn, U, u):
     return {"all": a64, "connected": c64}
 
 
-def check_parity(oracle_mod, gpu, Gup, Gdn, U, u, which, ref64=None):
+def check_parity(oracle_mod, gpu, Gup, Gdn, U, u, which, ref64=None, max_fraction=MAX_EXCEPTION_FRACTION, label=""):
     """gpu: float64 [B] from the CUDA path.  Returns a dict of statistics; raises AssertionError."""
     gpu = np.asarray(gpu, dtype=np.float64)
     B = gpu.shape[0]
@@ -36,11 +45,13 @@ def check_parity(oracle_mod, gpu, Gup, Gdn, U, u, which, ref64=None):
     diff = np.abs(gpu - ref64)
     ok = diff <= REL_TOL * scale
     bad = np.nonzero(~ok)[0]
-    stats = {"batch": B, "max_rel_strict": float((diff[ok] / np.maximum(scale[ok], 1e-300)).max()) if ok.any() else 0.0,
+    stats = {"label": label, "which": which, "n": int(Gup.shape[1]), "batch": B, "max_rel_strict": float((diff[ok] / np.maximum(scale[ok], 1e-300)).max()) if ok.any() else 0.0,
              "exceptions": int(bad.size), "worst_exception_sigmas": 0.0}
+    if not label.startswith("("):          # "(...)": a check that is expected to raise (tests of the rule itself)
+        STATS.append(stats)
     if bad.size == 0:
         return stats
-    assert bad.size <= max(1, int(MAX_EXCEPTION_FRACTION * B)), \
+    assert bad.size <= max(1, math.ceil(max_fraction * B)), \
         f"{which}: {bad.size}/{B} configurations miss the 1e-10 bar (max rel {float((diff / scale).max()):.3e})"
     # conditioning of the exceptions: relabelling scatter of the FP64 oracle around the long-double truth
     Gu = Gup[bad]
