@@ -51,6 +51,22 @@ def _load():
             f.restype = ctypes.c_int
             f.argtypes = [ctypes.c_int, ctypes.c_longlong, _c_double_p, _c_double_p, _c_double_p,
                           ctypes.c_double, _c_double_p, _c_double_p, ctypes.c_int]
+        for name in ("oracle_eval_lw", "oracle_eval_lw_f80"):
+            f = getattr(lib, name)
+            f.restype = ctypes.c_int
+            f.argtypes = [ctypes.c_int, ctypes.c_longlong, _c_double_p, _c_double_p, _c_double_p,
+                          ctypes.c_double, ctypes.c_double, _c_double_p, _c_double_p, ctypes.c_int]
+        lib.oracle_eval_halfvertex.restype = ctypes.c_int
+        lib.oracle_eval_halfvertex.argtypes = [ctypes.c_int, ctypes.c_longlong, _c_double_p, _c_double_p,
+                                               ctypes.c_double, _c_double_p, _c_double_p, ctypes.c_int]
+        lib.oracle_bruteforce_lw.restype = ctypes.c_int
+        lib.oracle_bruteforce_lw.argtypes = [ctypes.c_int, _c_double_p, _c_double_p, _c_double_p, ctypes.c_double,
+                                             _c_double_p, _c_double_p, ctypes.POINTER(ctypes.c_longlong)]
+        lib.oracle_bruteforce_halfvertex.restype = ctypes.c_int
+        lib.oracle_bruteforce_halfvertex.argtypes = [ctypes.c_int, _c_double_p, _c_double_p, ctypes.c_double,
+                                                     _c_double_p, _c_double_p, ctypes.POINTER(ctypes.c_longlong)]
+        lib.oracle_minors_lw.restype = None
+        lib.oracle_minors_lw.argtypes = [ctypes.c_int, _c_double_p, ctypes.c_double, _c_double_p]
         lib.oracle_minors.restype = None
         lib.oracle_minors.argtypes = [ctypes.c_int, _c_double_p, _c_double_p]
         lib.oracle_DC.restype = None
@@ -101,7 +117,7 @@ def build_G(xy, tau, table_up, table_dn, beta, g_diag=0.0):
     return Gup, Gdn
 
 
-def _eval(fname, Gup, Gdn, U, u, threads):
+def _eval(fname, Gup, Gdn, U, u, threads, loop_weight=None):
     lib = _load()
     Gup = _f64(Gup)
     Gdn = Gup if Gdn is None else _f64(Gdn)
@@ -114,8 +130,11 @@ def _eval(fname, Gup, Gdn, U, u, threads):
         up = _p(u)
     out_all = np.empty(B, dtype=np.float64)
     out_conn = np.empty(B, dtype=np.float64)
-    used = getattr(lib, fname)(n, B, _p(Gup), _p(Gdn), up, float(U), _p(out_all), _p(out_conn),
-                               int(threads))
+    if loop_weight is None:
+        used = getattr(lib, fname)(n, B, _p(Gup), _p(Gdn), up, float(U), _p(out_all), _p(out_conn), int(threads))
+    else:
+        used = getattr(lib, fname)(n, B, _p(Gup), _p(Gdn), up, float(U), float(loop_weight), _p(out_all),
+                                   _p(out_conn), int(threads))
     return out_all, out_conn, used
 
 
@@ -134,6 +153,58 @@ def eval_all_connected_f80(Gup, Gdn=None, U=1.0, u=None, threads=0):
     """Long-double accumulators ("truth" for conditioning reports)."""
     a, c, _ = _eval("oracle_eval_f80", Gup, Gdn, U, u, threads)
     return a, c
+
+
+def eval_all_connected_lw(Gup, Gdn=None, U=1.0, u=None, loop_weight=1.0, threads=0, f80=False):
+    """Loop-weight generalisation (reading R17): every closed fermion loop contributes -loop_weight."""
+    a, c, _ = _eval("oracle_eval_lw_f80" if f80 else "oracle_eval_lw", Gup, Gdn, U, u, threads, loop_weight)
+    return a, c
+
+
+def eval_halfvertex(W, V, loop_weight=1.0, threads=0):
+    """Half-vertex formulation (reading R18).  W [B, 2n', 2n'], V [B, n'].  Returns (all[B], connected[B])."""
+    lib = _load()
+    W, V = _f64(W), _f64(V)
+    B, m, m2 = W.shape
+    assert m == m2 and m % 2 == 0 and V.shape == (B, m // 2) and m <= 20
+    out_all = np.empty(B, dtype=np.float64)
+    out_conn = np.empty(B, dtype=np.float64)
+    lib.oracle_eval_halfvertex(m // 2, B, _p(W), _p(V), float(loop_weight), _p(out_all), _p(out_conn), int(threads))
+    return out_all, out_conn
+
+
+def bruteforce_lw(Gup, Gdn, u, loop_weight):
+    """Plain definition with (-loop_weight)^(closed loops), n <= 8.  Returns (all, connected, count)."""
+    lib = _load()
+    Gup, Gdn, u = _f64(Gup), _f64(Gdn), _f64(u)
+    a, c, k = ctypes.c_double(), ctypes.c_double(), ctypes.c_longlong()
+    rc = lib.oracle_bruteforce_lw(Gup.shape[0], _p(Gup), _p(Gdn), _p(u), float(loop_weight), ctypes.byref(a),
+                                  ctypes.byref(c), ctypes.byref(k))
+    if rc != 0:
+        raise ValueError("bruteforce_lw: n out of range")
+    return a.value, c.value, k.value
+
+
+def bruteforce_halfvertex(W, V, loop_weight=1.0):
+    """Plain definition of the half-vertex formulation, n' <= 4.  Returns (all, connected, count)."""
+    lib = _load()
+    W, V = _f64(W), _f64(V)
+    a, c, k = ctypes.c_double(), ctypes.c_double(), ctypes.c_longlong()
+    rc = lib.oracle_bruteforce_halfvertex(V.shape[0], _p(W), _p(V), float(loop_weight), ctypes.byref(a),
+                                          ctypes.byref(c), ctypes.byref(k))
+    if rc != 0:
+        raise ValueError("bruteforce_halfvertex: n' out of range")
+    return a.value, c.value, k.value
+
+
+def minors_lw(W, loop_weight):
+    """Z[S] = sum over permutations of S of (-loop_weight)^cyc prod W, for every subset S."""
+    lib = _load()
+    W = _f64(W)
+    n = W.shape[0]
+    Z = np.empty(1 << n, dtype=np.float64)
+    lib.oracle_minors_lw(n, _p(W), float(loop_weight), _p(Z))
+    return Z
 
 
 def minors(W):

@@ -94,8 +94,8 @@ void oracle_build_G(int n, long long batch, const int *xy, const double *tau,
  * out_all, out_connected: [batch] (either may be NULL).  threads <= 0: all OpenMP threads.
  * Returns the number of threads used.
  */
-int oracle_eval(int n, long long batch, const double *Gup, const double *Gdn,
-                const double *u, double U, double *out_all, double *out_connected, int threads)
+int oracle_eval_lw(int n, long long batch, const double *Gup, const double *Gdn, const double *u, double U,
+                   double loop_weight, double *out_all, double *out_connected, int threads)
 {
     int used = 1;
 #ifdef _OPENMP
@@ -112,7 +112,7 @@ int oracle_eval(int n, long long batch, const double *Gup, const double *Gdn,
         for (long long b = 0; b < batch; ++b) {
             for (int a = 0; a < n; ++a) ubuf[a] = u ? u[(size_t)b * n + a] : U;
             double all, conn;
-            eval_one_f64(n, Gup + (size_t)b * n * n, Gdn + (size_t)b * n * n, ubuf, work, &all, &conn);
+            eval_one_f64(n, Gup + (size_t)b * n * n, Gdn + (size_t)b * n * n, ubuf, -loop_weight, work, &all, &conn);
             if (out_all) out_all[b] = all;
             if (out_connected) out_connected[b] = conn;
         }
@@ -121,9 +121,16 @@ int oracle_eval(int n, long long batch, const double *Gup, const double *Gdn,
     return used;
 }
 
+/* The paper's own weight: -1 per closed fermion loop, i.e. loop_weight = 1. */
+int oracle_eval(int n, long long batch, const double *Gup, const double *Gdn,
+                const double *u, double U, double *out_all, double *out_connected, int threads)
+{
+    return oracle_eval_lw(n, batch, Gup, Gdn, u, U, 1.0, out_all, out_connected, threads);
+}
+
 /* Same, every accumulator in long double; results rounded to double on output ("truth" mode). */
-int oracle_eval_f80(int n, long long batch, const double *Gup, const double *Gdn,
-                    const double *u, double U, double *out_all, double *out_connected, int threads)
+int oracle_eval_lw_f80(int n, long long batch, const double *Gup, const double *Gdn, const double *u, double U,
+                       double loop_weight, double *out_all, double *out_connected, int threads)
 {
     int used = 1;
 #ifdef _OPENMP
@@ -140,7 +147,7 @@ int oracle_eval_f80(int n, long long batch, const double *Gup, const double *Gdn
         for (long long b = 0; b < batch; ++b) {
             for (int a = 0; a < n; ++a) ubuf[a] = u ? u[(size_t)b * n + a] : U;
             long double all, conn;
-            eval_one_f80(n, Gup + (size_t)b * n * n, Gdn + (size_t)b * n * n, ubuf, work, &all, &conn);
+            eval_one_f80(n, Gup + (size_t)b * n * n, Gdn + (size_t)b * n * n, ubuf, -loop_weight, work, &all, &conn);
             if (out_all) out_all[b] = (double)all;
             if (out_connected) out_connected[b] = (double)conn;
         }
@@ -149,12 +156,47 @@ int oracle_eval_f80(int n, long long batch, const double *Gup, const double *Gdn
     return used;
 }
 
-/* Z[S] for every subset S of one n x n matrix W (step 1 alone).  Z: [2^n]. */
-void oracle_minors(int n, const double *W, double *Z)
+int oracle_eval_f80(int n, long long batch, const double *Gup, const double *Gdn,
+                    const double *u, double U, double *out_all, double *out_connected, int threads)
+{
+    return oracle_eval_lw_f80(n, batch, Gup, Gdn, u, U, 1.0, out_all, out_connected, threads);
+}
+
+/* Z[S] for every subset S of one n x n matrix W (step 1 alone) with loop factor -loop_weight.  Z: [2^n]. */
+void oracle_minors_lw(int n, const double *W, double loop_weight, double *Z)
 {
     double *A = (double *)malloc(sizeof(double) * ((size_t)n << n));
-    propagate_f64(n, W, -1.0, Z, A);
+    propagate_f64(n, W, -loop_weight, Z, A);
     free(A);
+}
+
+void oracle_minors(int n, const double *W, double *Z) { oracle_minors_lw(n, W, 1.0, Z); }
+
+/* Half-vertex formulation (cos_oracle_core.inc: eval_one_halfvertex).  W: [batch][2n'][2n'], V: [batch][n']. */
+int oracle_eval_halfvertex(int np, long long batch, const double *W, const double *V, double loop_weight,
+                           double *out_all, double *out_connected, int threads)
+{
+    const int m = 2 * np;
+    int used = 1;
+#ifdef _OPENMP
+    if (threads <= 0) threads = omp_get_max_threads();
+    used = threads;
+#pragma omp parallel num_threads(threads)
+#endif
+    {
+        double *work = (double *)malloc(sizeof(double) * work_reals_f64(m));
+#ifdef _OPENMP
+#pragma omp for schedule(static)
+#endif
+        for (long long b = 0; b < batch; ++b) {
+            double all, conn;
+            eval_one_halfvertex_f64(np, W + (size_t)b * m * m, V + (size_t)b * np, -loop_weight, work, &all, &conn);
+            if (out_all) out_all[b] = all;
+            if (out_connected) out_connected[b] = conn;
+        }
+        free(work);
+    }
+    return used;
 }
 
 /* D[S] and C[S] for every subset of one configuration (steps 1-3), for the exp/log pin. */
@@ -225,8 +267,8 @@ static int uf_find(int *parent, int x)
     return x;
 }
 
-int oracle_bruteforce(int n, const double *Gup, const double *Gdn, const double *u,
-                      double *out_all, double *out_connected, long long *n_connected)
+int oracle_bruteforce_lw(int n, const double *Gup, const double *Gdn, const double *u, double loop_weight,
+                         double *out_all, double *out_connected, long long *n_connected)
 {
     if (n < 1 || n > 8) return -1;
     int fact = 1;
@@ -247,7 +289,8 @@ int oracle_bruteforce(int n, const double *Gup, const double *Gdn, const double 
         }
         double pu = 1.0, pd = 1.0;
         for (int i = 0; i < n; ++i) { pu *= Gup[i * n + p[i]]; pd *= Gdn[i * n + p[i]]; }
-        const double sg = (cyc & 1) ? -1.0 : 1.0;      /* (-1)^{number of closed fermion loops} */
+        double sg = 1.0;                               /* (-loop_weight)^{number of closed fermion loops}; */
+        for (int c = 0; c < cyc; ++c) sg *= -loop_weight;   /* loop_weight = 1: the paper's -1 per loop */
         tu[idx] = sg * pu;
         td[idx] = sg * pd;
         ++idx;
@@ -279,6 +322,51 @@ int oracle_bruteforce(int n, const double *Gup, const double *Gdn, const double 
     if (n_connected) *n_connected = cnt;
     free(perm);
     free(tu);
+    return 0;
+}
+
+int oracle_bruteforce(int n, const double *Gup, const double *Gdn, const double *u,
+                      double *out_all, double *out_connected, long long *n_connected)
+{
+    return oracle_bruteforce_lw(n, Gup, Gdn, u, 1.0, out_all, out_connected, n_connected);
+}
+
+/* Plain definition of the half-vertex formulation (cos_oracle_core.inc: eval_one_halfvertex): every permutation
+ * of the m = 2n' half-vertices, (-loop_weight)^cycles, connectivity of the interaction-line graph tested with
+ * union-find.  n' <= 4 (8! = 40320 permutations).  n_connected: number of connected permutations. */
+int oracle_bruteforce_halfvertex(int np, const double *W, const double *V, double loop_weight,
+                                 double *out_all, double *out_connected, long long *n_connected)
+{
+    if (np < 1 || np > 4) return -1;
+    const int m = 2 * np;
+    int p[8];
+    for (int i = 0; i < m; ++i) p[i] = i;
+    long double sum_all = 0, sum_conn = 0;
+    long long cnt = 0;
+    do {
+        int seen[8] = {0}, cyc = 0;
+        for (int i = 0; i < m; ++i) {
+            if (seen[i]) continue;
+            ++cyc;
+            for (int j = i; !seen[j]; j = p[j]) seen[j] = 1;
+        }
+        double term = 1.0;
+        for (int c = 0; c < cyc; ++c) term *= -loop_weight;
+        for (int i = 0; i < m; ++i) term *= W[i * m + p[i]];
+        sum_all += term;
+        int parent[4], comps = np;
+        for (int k = 0; k < np; ++k) parent[k] = k;
+        for (int i = 0; i < m; ++i) {
+            const int r0 = uf_find(parent, i / 2), r1 = uf_find(parent, p[i] / 2);
+            if (r0 != r1) { parent[r0] = r1; --comps; }
+        }
+        if (comps == 1) { sum_conn += term; ++cnt; }
+    } while (next_permutation_int(p, m));
+    long double w = 1;
+    for (int k = 0; k < np; ++k) w *= -(long double)V[k];
+    if (out_all) *out_all = (double)(w * sum_all);
+    if (out_connected) *out_connected = (double)(w * sum_conn);
+    if (n_connected) *n_connected = cnt;
     return 0;
 }
 

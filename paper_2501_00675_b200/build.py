@@ -16,7 +16,7 @@ SOURCES = ["cos_api.cu", "cos_probe.cu"]
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
-    "-shared", "-Xcompiler", "-fPIC",
+    "-shared", "-Xcompiler", "-fPIC", "--split-compile", "0",      # ptxas of the kernel variants in parallel
 ]
 
 

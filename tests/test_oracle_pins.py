@@ -285,7 +285,7 @@ def test_exp_log_consistency(oracle_mod, n):
 
 
 # ------------------------------------------------------------------ independent fast route
-@pytest.mark.parametrize("n", [6, 8, 10])
+@pytest.mark.parametrize("n", [6, 8, 10, 12])
 def test_independent_lu_minor_route(oracle_mod, n):
     """D(S) from numpy LU determinants of principal submatrices (no CoS code), then the subset
     recursion written separately here in the 'sum over the complement' form."""
