@@ -107,6 +107,27 @@ int cos_eval_connected_xt_host(cos_ctx* ctx, int n, long long batch, const int* 
                                const double* h_tau, double g_diag, const double* h_u, double U,
                                double* h_out);
 
+/* Loop-weight generalisation (reading R17).  The paper multiplies by -1 on closing a
+ * fermion loop (section IV); with N_f degenerate flavours the flavour trace of every closed loop
+ * contributes a further factor N_f, so the loop factor becomes -N_f:
+ *   Z_s[S] = sum_{sigma in Sym(S)} (-N_f)^{cyc(sigma)} prod_{i in S} G_s[i][sigma(i)]   (N_f = 1: (-1)^{|S|} det G_s[S,S]).
+ * n_f may be any finite double (n_f = -1 turns every Z_s[S] into a permanent); it applies to every later
+ * cos_eval_* call of this ctx, both species, all orders.  Default 1.  COS_EINVAL for NaN or infinity. */
+int cos_set_loop_weight(cos_ctx* ctx, double n_f);
+
+/* Half-vertex ("2n'") formulation, one species (reading R18).  The n_lines interaction
+ * lines k = 0..n_lines-1 each join the half-vertices 2k and 2k+1 with the potential V_k ("interaction potentials
+ * V_ab"); one species of fermion lines runs over all m = 2 n_lines half-vertices:
+ *   all       = prod_k(-V_k) * sum_{sigma in S_m} (-N_f)^{cyc(sigma)} prod_i W[i][sigma(i)]
+ *   connected = the same sum over the sigma whose interaction-line graph (an edge {i/2, sigma(i)/2} for every i)
+ *               is connected.
+ * d_W: [batch][m][m] row-major FP64, d_V: [batch][n_lines]; connected != 0 selects `connected`, else `all`;
+ * d_out: [batch].  1 <= n_lines <= COS_MAX_ORDER / 2.  N_f is the ctx loop weight (cos_set_loop_weight).
+ * Served by the plain one-thread-per-node kernel (propagation over the m points, D'[P] over the subsets of lines,
+ * reduction over n_lines bits): correct for every size, not tuned. */
+int cos_eval_halfvertex(cos_ctx* ctx, int n_lines, long long batch, const double* d_W, const double* d_V,
+                        int connected, double* d_out);
+
 /* Cross-check switch: enable != 0 routes every later cos_eval_* call of this ctx, whatever the order, through the
  * plain one-thread-per-node kernel (the one orders 1..4 always use) instead of the tuned team / pair kernels; it
  * runs on the same device with the same arguments and is only slower.  The GPU tests use it to compare the tuned

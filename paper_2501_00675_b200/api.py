@@ -37,6 +37,8 @@ SIGNATURES = {
     "cos_eval_connected": (_int, [_vp, _int, _ll, _vp, _vp, _vp, _dbl, _vp]),
     "cos_eval_connected_xt": (_int, [_vp, _int, _ll, _vp, _vp, _dbl, _vp, _dbl, _vp]),
     "cos_eval_connected_xt_host": (_int, [_vp, _int, _ll, _vp, _vp, _dbl, _vp, _dbl, _vp]),
+    "cos_set_loop_weight": (_int, [_vp, _dbl]),
+    "cos_eval_halfvertex": (_int, [_vp, _int, _ll, _vp, _vp, _int, _vp]),
     "cos_debug_force_generic": (_int, [_vp, _int]),
     "cos_last_launch_count": (_int, [_vp]),
     "cos_last_kernel_name": (ctypes.c_char_p, [_vp]),
@@ -227,6 +229,17 @@ class Context:
             self._h, n, batch, self._host(h_xy, "i32", (batch, n, 2), "h_xy"), self._host(h_tau, "f64", (batch, n), "h_tau"),
             float(g_diag), self._host(h_u, "f64", (batch, n), "h_u", optional=True), float(U),
             self._host(h_out, "f64", (batch,), "h_out")))
+
+    def eval_halfvertex(self, d_W, d_V, d_out, connected: bool = True):
+        """Half-vertex formulation (include/cos.h: cos_eval_halfvertex).  d_W [B, 2n', 2n'], d_V [B, n']."""
+        batch, m = int(d_W.shape[0]), int(d_W.shape[1])
+        self._check(self._lib.cos_eval_halfvertex(
+            self._h, m // 2, batch, self._dev(d_W, "f64", (batch, m, m), "d_W"),
+            self._dev(d_V, "f64", (batch, m // 2), "d_V"), 1 if connected else 0, self._dev(d_out, "f64", (batch,), "d_out")))
+
+    def set_loop_weight(self, n_f: float = 1.0):
+        """-n_f per closed fermion loop (include/cos.h: cos_set_loop_weight); 1 is the paper's rule."""
+        self._check(self._lib.cos_set_loop_weight(self._h, float(n_f)))
 
     def force_generic(self, on: bool = True):
         """Cross-check switch (include/cos.h: cos_debug_force_generic)."""

@@ -33,6 +33,7 @@ struct cos_ctx {
     cudaStream_t copy_stream = nullptr;                          // host path: H2D of chunk k+1 behind the kernels of chunk k
     cudaEvent_t copy_done[2] = {nullptr, nullptr};
     // bookkeeping
+    double loop_weight = 1.0;       // N_f: every closed fermion loop contributes -N_f (cos_set_loop_weight)
     bool force_generic = false;     // cos_debug_force_generic: every order through eval_generic_kernel
     int last_launches = 0;
     const char* last_kernel = "none";
@@ -125,7 +126,7 @@ int do_eval(cos_ctx* c, int n, long long batch, const double* gup, const double*
     if (batch == 0) return COS_OK;
     EvalArgs a{};
     a.n = n; a.batch = batch; a.Gup = gup; a.Gdn = gdn; a.u = u; a.U = U; a.out = out;
-    a.connected = connected; a.off = c->off;
+    a.connected = connected; a.off = c->off; a.loopf = -c->loop_weight;
     if (c->force_generic) {
         // no tables: the generic kernel computes its indices on the fly
     } else if (uses_team(n)) {   // table image of this order, built on first use
@@ -306,6 +307,37 @@ int cos_eval_connected(cos_ctx* c, int n, long long batch, const double* d_Gup, 
     return do_eval(c, n, batch, d_Gup, d_Gdn, d_u, U, d_out, 1);
 }
 
+int cos_eval_halfvertex(cos_ctx* c, int n_lines, long long batch, const double* d_W, const double* d_V, int connected,
+                        double* d_out)
+{
+    if (!c || n_lines < 1 || 2 * n_lines > COS_MAX_ORDER || batch < 0) return COS_EINVAL;
+    if (batch > 0 && (!d_W || !d_V || !d_out)) return COS_EINVAL;
+    cudaSetDevice(c->device);
+    c->last_launches = 0;
+    if (batch == 0) return COS_OK;
+    const int m = 2 * n_lines;
+    EvalArgs a{};
+    a.n = m; a.batch = batch; a.Gup = d_W; a.Gdn = d_W; a.u = d_V; a.U = 0.0; a.out = d_out;
+    a.connected = connected != 0; a.off = c->off; a.loopf = -c->loop_weight; a.halfvertex = 1;
+    const size_t per_cta = generic_scratch_doubles(m, c->smem_optin);
+    if (per_cta) {
+        const int ctas = eval_max_ctas(batch, c->num_sms);
+        int rc = grow(c, (void**)&c->scratch, &c->scratch_bytes, per_cta * sizeof(double) * (size_t)ctas);
+        if (rc != COS_OK) return rc;
+        a.scratch = c->scratch;
+        a.scratch_stride = per_cta;
+    }
+    const bool t = timer_begin(c);
+    int launches = 0;
+    const char* name = nullptr;
+    cudaError_t e = dispatch_eval(a, c->stream, c->num_sms, c->smem_optin, /*force_generic=*/true, &launches, &name);
+    if (t) timer_end(c);
+    if (e != cudaSuccess) return fail_cuda(c, e);
+    c->last_launches += launches;
+    c->last_kernel = name;
+    return COS_OK;
+}
+
 int cos_eval_connected_xt(cos_ctx* c, int n, long long batch, const int* d_xy, const double* d_tau,
                           double g_diag, const double* d_u, double U, double* d_out)
 {
@@ -380,6 +412,13 @@ int cos_eval_connected_xt_host(cos_ctx* c, int n, long long batch, const int* h_
 
 int cos_internal_device(const cos_ctx* c) { return c->device; }
 void* cos_internal_stream(const cos_ctx* c) { return (void*)c->stream; }
+
+int cos_set_loop_weight(cos_ctx* c, double n_f)
+{
+    if (!c || !(n_f == n_f) || n_f - n_f != 0.0) return COS_EINVAL;   // NaN / infinity
+    c->loop_weight = n_f;
+    return COS_OK;
+}
 
 int cos_debug_force_generic(cos_ctx* c, int enable)
 {

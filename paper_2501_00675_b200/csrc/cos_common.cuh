@@ -34,6 +34,9 @@ struct EvalArgs {
     double U;
     double* out;           // [batch]
     int connected;         // 0: D[full] ("all"), 1: C[full]
+    int halfvertex;        // 1: half-vertex formulation (reading R18): n = 2n' points, one species, u = V [batch][n'];
+                           //    generic kernel only
+    double loopf;          // factor of one closed fermion loop: -1, or -N_f (cos_set_loop_weight, reading R17)
     const uint32_t* off;   // off[R] = sum_{x<R}(popc(x)+1), R = 0..2^(kMaxN-1)
     double* scratch;       // per-CTA global scratch (large n), may be nullptr
     size_t scratch_stride; // doubles per CTA

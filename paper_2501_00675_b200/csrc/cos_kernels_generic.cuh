@@ -127,7 +127,8 @@ __global__ void __launch_bounds__(kThreads) eval_generic_kernel(EvalArgs a, int 
         __syncthreads();
         // ---- load W (both species) and the couplings; fold -u_a into the rows of W_up when the
         //      species are distinct (each term has exactly one factor from every row of S) ----
-        for (int t = tid; t < n; t += kThreads) uvec[t] = -(a.u ? a.u[b * n + t] : a.U);
+        const int nu = a.halfvertex ? n / 2 : n;             // couplings: per vertex, or per interaction line (R18)
+        for (int t = tid; t < nu; t += kThreads) uvec[t] = -(a.u ? a.u[b * nu + t] : a.U);
         __syncthreads();
         for (int t = tid; t < n * n; t += kThreads) {
             const double g = a.Gup[b * n * n + t];
@@ -157,7 +158,7 @@ __global__ void __launch_bounds__(kThreads) eval_generic_kernel(EvalArgs a, int 
                             double acc = ah * Ws[h * n + h];
                             unsigned m = R; int i = 0;
                             while (m) { const int c = __ffs(m) - 1; m &= m - 1; acc = fma(pr[i++], Ws[c * n + h], acc); }
-                            Zs[R | NR] = -acc;
+                            Zs[R | NR] = a.loopf * acc;            // -1 per closed fermion loop, -N_f in general (R17)
                         }
                         // extend to every c' < h not in R
                         unsigned absent = ~R & (NR - 1);
@@ -180,26 +181,41 @@ __global__ void __launch_bounds__(kThreads) eval_generic_kernel(EvalArgs a, int 
         if (!a.connected) {                                  // a5 "all": D[full]
             if (tid == 0) {
                 double w = 1.0;
-                if (nsp == 1) for (int v = 0; v < n; ++v) w *= uvec[v];
-                a.out[b] = w * Zup[N - 1] * Zdn[N - 1];
+                if (nsp == 1) for (int v = 0; v < nu; ++v) w *= uvec[v];
+                a.out[b] = w * Zup[N - 1] * (a.halfvertex ? 1.0 : Zdn[N - 1]);
             }
             continue;
         }
 
-        // ---- a3: D[S] = w(S) Zup[S] Zdn[S], stored over Zup ----
+        // ---- a3: D[S] = w(S) Zup[S] Zdn[S], stored over Zup.  Half-vertex formulation (R18): the reduction runs
+        //      over the n' interaction lines, D'[P] = prod_{k in P}(-V_k) Z[both half-vertices of every line of P],
+        //      stored in the (now free) frontier area ----
+        int nr = n;                                          // bits of the reduction
         double* D = Z;
-        for (unsigned S = tid; S < N; S += kThreads) {
-            double w = 1.0;
-            if (nsp == 1) { unsigned m = S; while (m) { const int v = __ffs(m) - 1; m &= m - 1; w *= uvec[v]; } }
-            D[S] = w * Zup[S] * Zdn[S];
+        double* C = P;
+        if (a.halfvertex) {
+            nr = n / 2;
+            D = P;
+            C = P + ((size_t)1 << nr);
+            for (unsigned Pm = tid; Pm < (1u << nr); Pm += kThreads) {
+                double w = 1.0;
+                unsigned S = 0, m = Pm;
+                while (m) { const int k = __ffs(m) - 1; m &= m - 1; w *= uvec[k]; S |= 3u << (2 * k); }
+                D[Pm] = w * Zup[S];
+            }
+        } else {
+            for (unsigned S = tid; S < N; S += kThreads) {
+                double w = 1.0;
+                if (nsp == 1) { unsigned m = S; while (m) { const int v = __ffs(m) - 1; m &= m - 1; w *= uvec[v]; } }
+                D[S] = w * Zup[S] * Zdn[S];
+            }
         }
         __syncthreads();
 
         // ---- a4: C'[S'] = D[2S'+1] - sum_{T' proper subset of S'} C'[T'] D[2(S'\T')], levels |S'| ----
-        double* C = P;
-        const unsigned M = N >> 1;                           // subsets of vertices 1..n-1
+        const unsigned M = 1u << (nr - 1);                   // subsets of vertices (lines) 1..nr-1
         const int lane = tid & 31, warp = tid >> 5, nwarps = kThreads >> 5;
-        for (int l = 0; l < n; ++l) {
+        for (int l = 0; l < nr; ++l) {
             if (l < 5) {
                 for (unsigned Sp = tid; Sp < M; Sp += kThreads) {
                     if (__popc(Sp) != l) continue;

@@ -124,6 +124,7 @@ inline PairDims pair_dims_global(int n, int threads, int nsp = 1)
 
 // Uniform description of one level step.
 struct PairLevel {
+    double lf;                  // factor of one closed loop (EvalArgs::loopf)
     int n, j;
     int cnt, cnt_next;          // patterns at levels j and j + 1
     int lvlZ_j, lvlZ_j1;        // Z record offsets of |S_Q| = j and j + 1
@@ -334,7 +335,7 @@ __device__ __forceinline__ void pair_item(const PairLevel& L, unsigned SQ, int x
         if (orec[k] < 0) continue;
         pair_store_rec<C>(sm + L.off_nxt, orec[k], acc[0][k], acc[1][k], acc[2][k], acc[3][k]);
     }
-    if (last) pair_store_rec<C>(sm + L.off_z, L.lvlZ_j1 + x, -acc[0][N], -acc[1][N], -acc[2][N], -acc[3][N]);
+    if (last) pair_store_rec<C>(sm + L.off_z, L.lvlZ_j1 + x, L.lf * acc[0][N], L.lf * acc[1][N], L.lf * acc[2][N], L.lf * acc[3][N]);
 }
 
 template <int C, int NCMAX, int KSKIP, bool DSC>
@@ -372,7 +373,7 @@ __device__ __forceinline__ void pair_dispatch_item(const PairLevel& L, unsigned 
 // Z[(SQ = {}, R_T)] for the 8 subsets of T (stages h < 3), one thread per instance, in the propagation's own
 // order (start / extend / close).  Wl: W of this instance (any replica); zr: Z record 0 + 4g doubles.
 template <int C>
-__device__ __forceinline__ void pair_small_stages(const double* Wl, int n, double* zr)
+__device__ __forceinline__ void pair_small_stages(const double* Wl, int n, double* zr, double lf)
 {
     constexpr int WE = PairLayout<C>::WE;
     auto W = [&](int a, int b) { return Wl[(a * n + b) * WE]; };
@@ -381,15 +382,15 @@ __device__ __forceinline__ void pair_small_stages(const double* Wl, int n, doubl
     const double w20 = W(2, 0), w21 = W(2, 1), w22 = W(2, 2);
     double z[8];
     z[0] = 1.0;                                           // top node
-    z[1] = -w00;                                          // stage 0
-    z[2] = -w11;                                          // stage 1, R = {}
-    z[3] = -fma(w10, w01, z[1] * w11);                    // stage 1, R = {0}: nodes (R,0) = W[1][0], (R,1) = Z[{0}]
-    z[4] = -w22;                                          // stage 2, R = {}
-    z[5] = -fma(w20, w02, z[1] * w22);                    // R = {0}
-    z[6] = -fma(w21, w12, z[2] * w22);                    // R = {1}
+    z[1] = lf * w00;                                      // stage 0 (lf: factor of one closed loop)
+    z[2] = lf * w11;                                      // stage 1, R = {}
+    z[3] = lf * fma(w10, w01, z[1] * w11);                // stage 1, R = {0}: nodes (R,0) = W[1][0], (R,1) = Z[{0}]
+    z[4] = lf * w22;                                      // stage 2, R = {}
+    z[5] = lf * fma(w20, w02, z[1] * w22);                // R = {0}
+    z[6] = lf * fma(w21, w12, z[2] * w22);                // R = {1}
     const double p01_1 = fma(w20, w01, z[1] * w21);       // node ({0,1}, 1) from R = {0}
     const double p01_0 = fma(w21, w10, z[2] * w20);       // node ({0,1}, 0) from R = {1}
-    z[7] = -fma(p01_0, w02, fma(p01_1, w12, z[3] * w22)); // R = {0,1}
+    z[7] = lf * fma(p01_0, w02, fma(p01_1, w12, z[3] * w22)); // R = {0,1}
 #pragma unroll
     for (int uu = 0; uu < 2; ++uu)
 #pragma unroll
@@ -521,13 +522,13 @@ __global__ void __launch_bounds__(MAXT, MINB) eval_pair_kernel(EvalArgs a, PairD
             team_prefetch_inputs<C>(a, n, nsp, stage, nx0, (int)min((long long)C, total_inst - nx0), tid, nthreads);
         }
         COS_PHASE_MARK(0);
-        if (tid < ninst) pair_small_stages<C>(smd + d.off_w + tid, n, rb + d.off_z + tid * 4);
+        if (tid < ninst) pair_small_stages<C>(smd + d.off_w + tid, n, rb + d.off_z + tid * 4, a.loopf);
         __syncthreads();
         COS_PHASE_MARK(1);
 
         // ---- a2: all stages together, level j = |S_Q| - 1; level j reads buffer (j & 1) and writes the other ----
         PairLevel L;
-        L.n = n; L.rank16 = rank16; L.off_z = d.off_z; L.dsc = reinterpret_cast<const uint32_t*>(a.tabs);
+        L.n = n; L.rank16 = rank16; L.off_z = d.off_z; L.lf = a.loopf; L.dsc = reinterpret_cast<const uint32_t*>(a.tabs);
         for (int j = 0; j < qmax; ++j) {
             L.j = j;
             L.cnt = kBinom.c[qmax][j + 1];

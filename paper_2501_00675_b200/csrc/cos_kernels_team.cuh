@@ -131,6 +131,7 @@ inline TeamDims team_dims(int n, int nsp)
 
 // Uniform description of one level step.
 struct TeamLevel {
+    double lf;                  // factor of one closed loop (EvalArgs::loopf)
     int n, j;
     int cnt, cnt_next;          // patterns at levels j and j + 1
     int lvlZ_j, lvlZ_j1;        // Z record offsets of |S_Q| = j and j + 1
@@ -284,7 +285,7 @@ __device__ __forceinline__ void team_item(const TeamLevel& L, const uint32_t* ds
             for (int t = 0; t < NT; ++t)
                 if ((t >> ts) & 1) acc[t][k] = fma(accT[t ^ (1 << ts)][ts], w, acc[t][k]);
         }
-    // ---- outputs: next-level records, and Z[(SQ, R_T)] = -close (one -1 per closed fermion loop) ----
+    // ---- outputs: next-level records, and Z[(SQ, R_T)] = lf * close (lf = -1 per closed fermion loop) ----
 #pragma unroll
     for (int k = 0; k < N; ++k) {
         if (orec[k] == 0xffff) continue;
@@ -297,7 +298,7 @@ __device__ __forceinline__ void team_item(const TeamLevel& L, const uint32_t* ds
         const RecPtr<C> o(sm + L.off_z, L.lvlZ_j1 + x);
 #pragma unroll
         for (int p = 0; p < 4; ++p)
-            *reinterpret_cast<double2*>(o.part(p)) = make_double2(-acc[2 * p][N], -acc[2 * p + 1][N]);
+            *reinterpret_cast<double2*>(o.part(p)) = make_double2(L.lf * acc[2 * p][N], L.lf * acc[2 * p + 1][N]);
     }
 }
 
@@ -380,7 +381,7 @@ __device__ __forceinline__ void team_item_col(const TeamLevel& L, const uint32_t
         for (int t = 0; t < NT; ++t)
             if ((t >> ts) & 1) acc[t] = fma(accT[t ^ (1 << ts)][ts], w, acc[t]);
     }
-    const double sg = close ? -1.0 : 1.0;             // Z = -close (one -1 per closed fermion loop)
+    const double sg = close ? L.lf : 1.0;             // Z = lf * close (lf = -1 per closed fermion loop)
     const int orec = close ? L.lvlZ_j1 + x : (int)reinterpret_cast<const uint16_t*>(dsc + 1)[k];
     const RecPtr<C> o(sm + (close ? L.off_z : L.off_nxt), orec);
 #pragma unroll
@@ -410,7 +411,7 @@ __device__ __forceinline__ void team_dispatch_item(const TeamLevel& L, const uin
 // Z[(SQ = {}, R_T)] for the 8 subsets of T (stages h < 3), one thread per instance, in the propagation's own
 // order (start / extend / close).  zr points at Z record 0 of this instance (already offset by g * 2).
 template <int C>
-__device__ __forceinline__ void team_small_stages(const double* Wl, int n, double* zr)
+__device__ __forceinline__ void team_small_stages(const double* Wl, int n, double* zr, double lf)
 {
     using Lay = TeamLayout<C>;
     constexpr int WE = Lay::WE, PART = Lay::PART;
@@ -420,15 +421,15 @@ __device__ __forceinline__ void team_small_stages(const double* Wl, int n, doubl
     const double w20 = W(2, 0), w21 = W(2, 1), w22 = W(2, 2);
     double z[8];
     z[0] = 1.0;                                           // top node
-    z[1] = -w00;                                          // stage 0
-    z[2] = -w11;                                          // stage 1, R = {}
-    z[3] = -fma(w10, w01, z[1] * w11);                    // stage 1, R = {0}: nodes (R,0) = W[1][0], (R,1) = Z[{0}]
-    z[4] = -w22;                                          // stage 2, R = {}
-    z[5] = -fma(w20, w02, z[1] * w22);                    // R = {0}
-    z[6] = -fma(w21, w12, z[2] * w22);                    // R = {1}
+    z[1] = lf * w00;                                      // stage 0 (lf: factor of one closed loop)
+    z[2] = lf * w11;                                      // stage 1, R = {}
+    z[3] = lf * fma(w10, w01, z[1] * w11);                // stage 1, R = {0}: nodes (R,0) = W[1][0], (R,1) = Z[{0}]
+    z[4] = lf * w22;                                      // stage 2, R = {}
+    z[5] = lf * fma(w20, w02, z[1] * w22);                // R = {0}
+    z[6] = lf * fma(w21, w12, z[2] * w22);                // R = {1}
     const double p01_1 = fma(w20, w01, z[1] * w21);       // node ({0,1}, 1) from R = {0}
     const double p01_0 = fma(w21, w10, z[2] * w20);       // node ({0,1}, 0) from R = {1}
-    z[7] = -fma(p01_0, w02, fma(p01_1, w12, z[3] * w22)); // R = {0,1}
+    z[7] = lf * fma(p01_0, w02, fma(p01_1, w12, z[3] * w22)); // R = {0,1}
 #pragma unroll
     for (int t = 0; t < 8; t += 2) *reinterpret_cast<double2*>(zr + (t >> 1) * PART) = make_double2(z[t], z[t + 1]);   // record 0: no swizzle
 }
@@ -956,13 +957,13 @@ __global__ void __launch_bounds__(MAXT, MINB) eval_team_kernel(EvalArgs a, TeamD
         __syncthreads();          // W of this team is in place; the previous team's last reads are done
         team_set_couplings<C>(a, n, nsp, stage, smd + d.off_u, ninst, tid, nthreads);
         COS_PHASE_MARK_T(0, nthreads);
-        if (tid < ninst) team_small_stages<C>(smd + d.off_w + tid, n, smd + d.off_z + tid * 2);
+        if (tid < ninst) team_small_stages<C>(smd + d.off_w + tid, n, smd + d.off_z + tid * 2, a.loopf);
         team_sync(nthreads);
         COS_PHASE_MARK_T(1, nthreads);
 
         // ---- a2: all stages together, level j = |S_Q| - 1 ----
         TeamLevel L;
-        L.n = n; L.rank16 = rank16; L.off_z = d.off_z;
+        L.n = n; L.rank16 = rank16; L.off_z = d.off_z; L.lf = a.loopf;
         int cur = d.off_b0, nxt = d.off_b1;
         for (int j = 0; j < qmax; ++j) {
             L.j = j;

@@ -29,18 +29,19 @@ CLUSTERED_EXCEPTION_FRACTION = 0.01
 STATS = []          # one dict per check_parity call (label, batch, exceptions, ...)
 
 
-def oracle_reference(oracle_mod, Gup, Gdn, U, u):
-    a64, c64 = oracle_mod.eval_all_connected(Gup, Gdn, U=U, u=u)
+def oracle_reference(oracle_mod, Gup, Gdn, U, u, loop_weight=1.0):
+    a64, c64 = oracle_mod.eval_all_connected_lw(Gup, Gdn, U=U, u=u, loop_weight=loop_weight)
     return {"all": a64, "connected": c64}
 
 
-def check_parity(oracle_mod, gpu, Gup, Gdn, U, u, which, ref64=None, max_fraction=MAX_EXCEPTION_FRACTION, label=""):
+def check_parity(oracle_mod, gpu, Gup, Gdn, U, u, which, ref64=None, max_fraction=MAX_EXCEPTION_FRACTION, label="",
+                 loop_weight=1.0):
     """gpu: float64 [B] from the CUDA path.  Returns a dict of statistics; raises AssertionError."""
     gpu = np.asarray(gpu, dtype=np.float64)
     B = gpu.shape[0]
     assert np.all(np.isfinite(gpu)), "non-finite GPU result"
     if ref64 is None:
-        ref64 = oracle_reference(oracle_mod, Gup, Gdn, U, u)[which]
+        ref64 = oracle_reference(oracle_mod, Gup, Gdn, U, u, loop_weight)[which]
     scale = np.abs(ref64)
     diff = np.abs(gpu - ref64)
     ok = diff <= REL_TOL * scale
@@ -58,7 +59,8 @@ def check_parity(oracle_mod, gpu, Gup, Gdn, U, u, which, ref64=None, max_fractio
     Gd = Gu if Gdn is None else Gdn[bad]
     uu = None if u is None else u[bad]
     pick = 0 if which == "all" else 1
-    truth = oracle_mod.eval_all_connected_f80(Gu, None if Gdn is None else Gd, U=U, u=uu)[pick]
+    truth = oracle_mod.eval_all_connected_lw(Gu, None if Gdn is None else Gd, U=U, u=uu, loop_weight=loop_weight,
+                                             f80=True)[pick]
     n = Gup.shape[1]
     rng = np.random.default_rng(12345)
     dev2 = np.zeros(bad.size)
@@ -67,7 +69,7 @@ def check_parity(oracle_mod, gpu, Gup, Gdn, U, u, which, ref64=None, max_fractio
         Gu_p = np.ascontiguousarray(Gu[:, p][:, :, p])
         Gd_p = None if Gdn is None else np.ascontiguousarray(Gd[:, p][:, :, p])
         uu_p = None if uu is None else np.ascontiguousarray(uu[:, p])
-        v = oracle_mod.eval_all_connected(Gu_p, Gd_p, U=U, u=uu_p)[pick]
+        v = oracle_mod.eval_all_connected_lw(Gu_p, Gd_p, U=U, u=uu_p, loop_weight=loop_weight)[pick]
         dev2 += (v - truth) ** 2
     sigma = np.sqrt(dev2 / K_RELABEL)
     err = np.abs(gpu[bad] - truth)

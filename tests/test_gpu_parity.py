@@ -293,3 +293,53 @@ def test_generic_kernel_cross_check(torch_mod, oracle_mod, n):
         np.testing.assert_allclose(got, tuned, rtol=1e-9)
         got1 = _gpu_eval(torch_mod, c, Gup, None, 1.3, None, "connected")
         check_parity(oracle_mod, got1, Gup, None, 1.3, None, "connected", label="forced generic kernel aliased")
+
+
+# ------------------------------------------------------------------------------------------ f3: loop weight
+@pytest.mark.parametrize("n", [2, 4, 6, 9, 10, 11, 12, 13, 14])
+def test_loop_weight(torch_mod, oracle_mod, n):
+    """cos_set_loop_weight: -N_f per closed fermion loop (reading R17) through every kernel family, one and two
+    species, against the oracle's loop-weight mode; N_f = 1 restores the default."""
+    from paper_2501_00675_b200 import api
+    rng = np.random.default_rng(4000 + n)
+    B = 45 if n <= 12 else 5
+    Gup = rng.normal(size=(B, n, n)) / np.sqrt(n) + 0.5 * np.eye(n)
+    Gdn = rng.normal(size=(B, n, n)) / np.sqrt(n) + 0.5 * np.eye(n)
+    u = rng.uniform(0.5, 2.0, size=(B, n))
+    with api.Context() as c:
+        for nf in (2.0, -1.0, 0.5):
+            c.set_loop_weight(nf)
+            for which in ("all", "connected"):
+                got = _gpu_eval(torch_mod, c, Gup, Gdn, 1.0, u, which)
+                check_parity(oracle_mod, got, Gup, Gdn, 1.0, u, which, loop_weight=nf, label=f"loop weight {nf}")
+            got = _gpu_eval(torch_mod, c, Gup, None, 1.3, None, "connected")
+            check_parity(oracle_mod, got, Gup, None, 1.3, None, "connected", loop_weight=nf,
+                         label=f"loop weight {nf} aliased")
+        c.set_loop_weight(1.0)
+        got = _gpu_eval(torch_mod, c, Gup, Gdn, 1.0, u, "connected")
+        check_parity(oracle_mod, got, Gup, Gdn, 1.0, u, "connected", label="loop weight reset")
+
+
+@pytest.mark.parametrize("nl", [1, 2, 3, 4, 5, 6, 7])
+def test_halfvertex(torch_mod, oracle_mod, nl):
+    """cos_eval_halfvertex (reading R18) against the oracle's half-vertex mode, N_f = 1 and 2."""
+    from paper_2501_00675_b200 import api
+    torch = torch_mod
+    m = 2 * nl
+    rng = np.random.default_rng(6000 + nl)
+    B = 333 if nl <= 5 else 19                        # more configurations than persistent CTAs at small sizes
+    W = rng.normal(size=(B, m, m)) / np.sqrt(m) + 0.5 * np.eye(m)
+    V = rng.uniform(0.5, 2.0, size=(B, nl))
+    with api.Context() as c:
+        for nf in (1.0, 2.0):
+            c.set_loop_weight(nf)
+            ref_all, ref_conn = oracle_mod.eval_halfvertex(W, V, loop_weight=nf)
+            for connected, ref in ((False, ref_all), (True, ref_conn)):
+                out = torch.empty(B, dtype=torch.float64, device="cuda")
+                c.eval_halfvertex(_dev(torch, W), _dev(torch, V), out, connected=connected)
+                torch.cuda.synchronize()
+                assert c.last_kernel_name() == "eval_generic_kernel" and c.last_launch_count() >= 1
+                got = out.cpu().numpy()
+                bad = np.abs(got - ref) > 1e-10 * np.abs(ref)
+                assert bad.sum() <= max(1, int(np.ceil(2e-3 * B))), (nl, nf, connected, np.abs(got / ref - 1).max())
+                assert np.all(np.abs(got - ref) <= 1e-7 * np.abs(ref))
