@@ -82,6 +82,16 @@ def _load():
         lib.oracle_bruteforce.argtypes = [ctypes.c_int, _c_double_p, _c_double_p, _c_double_p,
                                           _c_double_p, _c_double_p,
                                           ctypes.POINTER(ctypes.c_longlong)]
+        lib.oracle_philox4x32_10.restype = None
+        lib.oracle_philox4x32_10.argtypes = [ctypes.POINTER(ctypes.c_uint32)] * 3
+        lib.oracle_u53.restype = ctypes.c_double
+        lib.oracle_u53.argtypes = [ctypes.c_uint32, ctypes.c_uint32]
+        lib.oracle_mc_run.restype = None
+        lib.oracle_mc_run.argtypes = [ctypes.c_int, ctypes.c_longlong, ctypes.c_int, ctypes.c_ulonglong, _c_int_p,
+                                      _c_double_p, _c_double_p, ctypes.c_int, ctypes.c_int, ctypes.c_int,
+                                      ctypes.c_double, ctypes.c_double, ctypes.c_double, ctypes.c_double, _c_double_p,
+                                      ctypes.POINTER(ctypes.c_ubyte), _c_double_p,
+                                      ctypes.POINTER(ctypes.c_longlong), _c_double_p, ctypes.c_int]
         lib.oracle_max_threads.restype = ctypes.c_int
         lib.oracle_max_threads.argtypes = []
         _lib = lib
@@ -264,3 +274,39 @@ def bruteforce(Gup, Gdn, u):
     if rc != 0:
         raise ValueError("bruteforce: n out of range")
     return a.value, c.value, k.value
+
+
+def philox4x32_10(counter, key):
+    """Counter-based generator of reading R19: counter (4 x uint32), key (2 x uint32) -> 4 x uint32."""
+    lib = _load()
+    c = (ctypes.c_uint32 * 4)(*[int(x) & 0xFFFFFFFF for x in counter])
+    k = (ctypes.c_uint32 * 2)(*[int(x) & 0xFFFFFFFF for x in key])
+    o = (ctypes.c_uint32 * 4)()
+    lib.oracle_philox4x32_10(c, k, o)
+    return tuple(int(x) for x in o)
+
+
+def u53(a, b):
+    return float(_load().oracle_u53(int(a) & 0xFFFFFFFF, int(b) & 0xFFFFFFFF))
+
+
+def mc_run(xy, tau, table, beta, steps, seed, U=1.0, g_diag=0.0, loop_weight=1.0, threads=0):
+    """Metropolis walkers of reading R19.  xy [W,n,2] int32, tau [W,n] (copied, not modified).  Returns a dict:
+    xy, tau (final state), weight [W], accept [steps,W] uint8, margin [steps,W], accepted [W], sign_sum [W]."""
+    lib = _load()
+    xy = np.array(xy, dtype=np.int32, order="C", copy=True)
+    tau = np.array(tau, dtype=np.float64, order="C", copy=True)
+    table = _f64(table)
+    W, n = tau.shape
+    Lx, Ly, ntau = table.shape
+    weight = np.empty(W)
+    hist = np.empty((steps, W), dtype=np.uint8)
+    margin = np.empty((steps, W))
+    accepted = np.empty(W, dtype=np.int64)
+    sign_sum = np.empty(W)
+    lib.oracle_mc_run(n, W, int(steps), int(seed), xy.ctypes.data_as(_c_int_p), _p(tau), _p(table), Lx, Ly, ntau,
+                      float(beta), float(g_diag), float(U), float(loop_weight), _p(weight),
+                      hist.ctypes.data_as(ctypes.POINTER(ctypes.c_ubyte)), _p(margin),
+                      accepted.ctypes.data_as(ctypes.POINTER(ctypes.c_longlong)), _p(sign_sum), int(threads))
+    return {"xy": xy, "tau": tau, "weight": weight, "accept": hist, "margin": margin, "accepted": accepted,
+            "sign_sum": sign_sum}

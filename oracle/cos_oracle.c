@@ -370,6 +370,106 @@ int oracle_bruteforce_halfvertex(int np, const double *W, const double *V, doubl
     return 0;
 }
 
+/* ------------------------------------------------------------------------------------------
+ * Monte Carlo over the vertex coordinates (reading R19).
+ * P:47 "The integration over the vertex coordinates can then be performed by stochastic (Monte Carlo) sampling";
+ * P:137 "one needs to handle proposal and acceptance of configurations ... readily implemented in device-sided
+ * code".  The paper gives no update scheme; reading R19 fixes the plainest one: independent Metropolis walkers
+ * ("many Markov chain walkers"), configuration weight |connected(x)|, one update per step:
+ *   draw (r0, r1, r2, r3) = philox4x32_10(counter = (step, 0, walker_lo, walker_hi), key = (seed_lo, seed_hi))
+ *   and  (s0, s1, s2, s3) = philox4x32_10(counter = (step, 1, walker_lo, walker_hi), same key);
+ *   vertex k = r0 mod n moves to site (r1 mod Lx, r2 mod Ly) and time beta * u53(s0, s1);
+ *   accept iff u53(s2, s3) * |w_old| < |w_new|   (symmetric proposal: min(1, |w_new| / |w_old|));
+ *   u53(a, b) = (((uint64)a << 21) ^ ((uint64)b >> 11)) * 2^-53 in [0, 1).
+ * philox4x32_10 is the counter-based generator of Salmon et al. (SC'11), restated here from its definition.
+ */
+typedef unsigned int u32;
+typedef unsigned long long u64;
+
+void oracle_philox4x32_10(const u32 ctr[4], const u32 key[2], u32 out[4])
+{
+    u32 c0 = ctr[0], c1 = ctr[1], c2 = ctr[2], c3 = ctr[3], k0 = key[0], k1 = key[1];
+    for (int round = 0; round < 10; ++round) {
+        const u64 p0 = (u64)0xD2511F53u * c0, p1 = (u64)0xCD9E8D57u * c2;
+        const u32 n0 = (u32)(p1 >> 32) ^ c1 ^ k0, n1 = (u32)p1;
+        const u32 n2 = (u32)(p0 >> 32) ^ c3 ^ k1, n3 = (u32)p0;
+        c0 = n0; c1 = n1; c2 = n2; c3 = n3;
+        k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;          /* Weyl key schedule */
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+double oracle_u53(u32 a, u32 b)
+{
+    const u64 x = ((u64)a << 21) ^ ((u64)b >> 11);
+    return (double)x * (1.0 / 9007199254740992.0);
+}
+
+/* xy [walkers][n][2], tau [walkers][n]: state, in/out.  weight [walkers]: connected value of the current
+ * configuration (out).  accept_hist: NULL or [steps][walkers] (1 = accepted).  margin: NULL or [steps][walkers],
+ * (|w_new| - r |w_old|) / max(|w_new|, |w_old|): a decision with |margin| below the parity tolerance is a tie that
+ * another FP64 evaluation order may take the other way.  accepted [walkers], sign_sum [walkers] (sum over the
+ * steps of sign(w) of the configuration held AFTER the step): out.  One table for both species (G_up = G_dn). */
+void oracle_mc_run(int n, long long walkers, int steps, u64 seed, int *xy, double *tau,
+                   const double *table, int Lx, int Ly, int ntau, double beta, double g_diag, double U,
+                   double loop_weight, double *weight, unsigned char *accept_hist, double *margin,
+                   long long *accepted, double *sign_sum, int threads)
+{
+#ifdef _OPENMP
+    if (threads <= 0) threads = omp_get_max_threads();
+#pragma omp parallel for num_threads(threads) schedule(static)
+#endif
+    for (long long w = 0; w < walkers; ++w) {
+        double *work = (double *)malloc(sizeof(double) * (work_reals_f64(n) + 2 * (size_t)n * n));
+        double *G = work + work_reals_f64(n);
+        int pxy[2 * 32];
+        double ptau[32], ubuf[32];
+        for (int a = 0; a < n; ++a) ubuf[a] = U;
+        int *sx = xy + (size_t)w * n * 2;
+        double *st = tau + (size_t)w * n;
+        double all, wold;
+        oracle_build_G(n, 1, sx, st, table, table, Lx, Ly, ntau, beta, g_diag, G, NULL);
+        eval_one_f64(n, G, G, ubuf, -loop_weight, work, &all, &wold);
+        long long acc = 0;
+        double ss = 0.0;
+        const u32 key[2] = {(u32)seed, (u32)(seed >> 32)};
+        for (int step = 0; step < steps; ++step) {
+            u32 r[4], s[4];
+            const u32 c0[4] = {(u32)step, 0u, (u32)w, (u32)((u64)w >> 32)};
+            const u32 c1[4] = {(u32)step, 1u, (u32)w, (u32)((u64)w >> 32)};
+            oracle_philox4x32_10(c0, key, r);
+            oracle_philox4x32_10(c1, key, s);
+            memcpy(pxy, sx, sizeof(int) * 2 * n);
+            memcpy(ptau, st, sizeof(double) * n);
+            const int k = (int)(r[0] % (u32)n);
+            pxy[2 * k] = (int)(r[1] % (u32)Lx);
+            pxy[2 * k + 1] = (int)(r[2] % (u32)Ly);
+            ptau[k] = beta * oracle_u53(s[0], s[1]);
+            double wnew;
+            oracle_build_G(n, 1, pxy, ptau, table, table, Lx, Ly, ntau, beta, g_diag, G, NULL);
+            eval_one_f64(n, G, G, ubuf, -loop_weight, work, &all, &wnew);
+            const double rr = oracle_u53(s[2], s[3]);
+            const int ok = rr * fabs(wold) < fabs(wnew);
+            if (margin) {
+                const double big = fabs(wold) > fabs(wnew) ? fabs(wold) : fabs(wnew);
+                margin[(size_t)step * walkers + w] = big > 0 ? (fabs(wnew) - rr * fabs(wold)) / big : 0.0;
+            }
+            if (ok) {
+                memcpy(sx, pxy, sizeof(int) * 2 * n);
+                memcpy(st, ptau, sizeof(double) * n);
+                wold = wnew;
+                ++acc;
+            }
+            if (accept_hist) accept_hist[(size_t)step * walkers + w] = (unsigned char)ok;
+            ss += (wold > 0) - (wold < 0);
+        }
+        weight[w] = wold;
+        if (accepted) accepted[w] = acc;
+        if (sign_sum) sign_sum[w] = ss;
+        free(work);
+    }
+}
+
 int oracle_max_threads(void)
 {
 #ifdef _OPENMP
