@@ -107,6 +107,27 @@ int cos_eval_connected_xt_host(cos_ctx* ctx, int n, long long batch, const int* 
                                const double* h_tau, double g_diag, const double* h_u, double U,
                                double* h_out);
 
+/* On-device Monte Carlo over the vertex coordinates (reading R19).
+ * (section II.B): "The integration over the vertex coordinates can then be performed by stochastic (Monte Carlo)
+ * sampling"; line 137 (section IV.A): "one needs to handle proposal and acceptance of configurations ... readily
+ * implemented in device-sided code"; line 87: "many Markov chain walkers".  Every configuration of the batch is an
+ * independent Metropolis walker with weight |connected|.  Step t of walker w draws
+ *   (r0..r3) = philox4x32_10(counter (t, 0, w_lo, w_hi), key (seed_lo, seed_hi)),  (s0..s3) = same with counter (t, 1, ..),
+ * moves vertex k = r0 mod n to site (r1 mod Lx, r2 mod Ly) and time beta * u53(s0, s1), and accepts iff
+ * u53(s2, s3) * |w_old| < |w_new|, with u53(a, b) = ((a << 21) ^ (b >> 11)) * 2^-53.  The proposals of all walkers
+ * are evaluated by one pass of the hot path (cos_build_G + evaluation kernel), so a step is four kernel launches
+ * and nothing crosses to the host.
+ *   d_xy [walkers][n][2], d_tau [walkers][n]: the walkers' configurations, updated in place;
+ *   d_weight [walkers]: connected value of the final configurations (out);
+ *   d_accept_hist: NULL or [steps][walkers], 1 where the proposal of that step was accepted;
+ *   d_accepted: NULL or [walkers] accepted proposals; d_sign_sum: NULL or [walkers], sum over the steps of the
+ *   sign of the weight held after the step (numerator of the average sign).
+ * Uses the table registered for both species (COS_EINVAL if two different tables are registered) and the ctx
+ * loop weight.  COS_ENOTABLE without a table. */
+int cos_mc_run(cos_ctx* ctx, int n, long long walkers, int steps, unsigned long long seed, int* d_xy, double* d_tau,
+               double g_diag, double U, double* d_weight, unsigned char* d_accept_hist, long long* d_accepted,
+               double* d_sign_sum);
+
 /* Loop-weight generalisation (reading R17).  The paper multiplies by -1 on closing a
  * fermion loop (section IV); with N_f degenerate flavours the flavour trace of every closed loop
  * contributes a further factor N_f, so the loop factor becomes -N_f:

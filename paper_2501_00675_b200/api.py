@@ -37,6 +37,7 @@ SIGNATURES = {
     "cos_eval_connected": (_int, [_vp, _int, _ll, _vp, _vp, _vp, _dbl, _vp]),
     "cos_eval_connected_xt": (_int, [_vp, _int, _ll, _vp, _vp, _dbl, _vp, _dbl, _vp]),
     "cos_eval_connected_xt_host": (_int, [_vp, _int, _ll, _vp, _vp, _dbl, _vp, _dbl, _vp]),
+    "cos_mc_run": (_int, [_vp, _int, _ll, _int, ctypes.c_ulonglong, _vp, _vp, _dbl, _dbl, _vp, _vp, _vp, _vp]),
     "cos_set_loop_weight": (_int, [_vp, _dbl]),
     "cos_eval_halfvertex": (_int, [_vp, _int, _ll, _vp, _vp, _int, _vp]),
     "cos_debug_force_generic": (_int, [_vp, _int]),
@@ -229,6 +230,28 @@ class Context:
             self._h, n, batch, self._host(h_xy, "i32", (batch, n, 2), "h_xy"), self._host(h_tau, "f64", (batch, n), "h_tau"),
             float(g_diag), self._host(h_u, "f64", (batch, n), "h_u", optional=True), float(U),
             self._host(h_out, "f64", (batch,), "h_out")))
+
+    def mc_run(self, d_xy, d_tau, d_weight, steps: int, seed: int, U: float = 1.0, g_diag: float = 0.0,
+               d_accept_hist=None, d_accepted=None, d_sign_sum=None):
+        """Metropolis walkers on the device (include/cos.h: cos_mc_run); d_xy / d_tau are updated in place."""
+        walkers, n = (int(s) for s in d_tau.shape)
+        hist = None
+        if d_accept_hist is not None:
+            k, shp = _kind(d_accept_hist)
+            if k != "uint8" or shp != (int(steps), walkers) or not d_accept_hist.is_cuda or not d_accept_hist.is_contiguous():
+                raise CosError(COS_EINVAL, "d_accept_hist: expected a contiguous CUDA uint8 tensor [steps, walkers]")
+            hist = _ptr(d_accept_hist)
+        acc = None
+        if d_accepted is not None:
+            k, shp = _kind(d_accepted)
+            if k != "int64" or shp != (walkers,) or not d_accepted.is_cuda or not d_accepted.is_contiguous():
+                raise CosError(COS_EINVAL, "d_accepted: expected a contiguous CUDA int64 tensor [walkers]")
+            acc = _ptr(d_accepted)
+        self._check(self._lib.cos_mc_run(
+            self._h, n, walkers, int(steps), int(seed), self._dev(d_xy, "i32", (walkers, n, 2), "d_xy"),
+            self._dev(d_tau, "f64", (walkers, n), "d_tau"), float(g_diag), float(U),
+            self._dev(d_weight, "f64", (walkers,), "d_weight"), hist, acc,
+            self._dev(d_sign_sum, "f64", (walkers,), "d_sign_sum", optional=True)))
 
     def eval_halfvertex(self, d_W, d_V, d_out, connected: bool = True):
         """Half-vertex formulation (include/cos.h: cos_eval_halfvertex).  d_W [B, 2n', 2n'], d_V [B, n']."""

@@ -11,6 +11,7 @@
 #include "cos_internal.h"
 #include "cos_kernels_generic.cuh"
 #include "cos_dispatch.cuh"
+#include "cos_mc.cuh"
 
 using namespace cosb;
 
@@ -30,6 +31,7 @@ struct cos_ctx {
     unsigned char* team_tabs[COS_MAX_ORDER + 1] = {};            // per order: table image of the team kernel / item
                                                                  // descriptors of the pair kernel
     void* stage = nullptr;          size_t stage_bytes = 0;      // device staging of the host path
+    void* mc = nullptr;             size_t mc_bytes = 0;         // cos_mc_run: proposal coordinates and weights
     cudaStream_t copy_stream = nullptr;                          // host path: H2D of chunk k+1 behind the kernels of chunk k
     cudaEvent_t copy_done[2] = {nullptr, nullptr};
     // bookkeeping
@@ -255,6 +257,7 @@ int cos_destroy(cos_ctx* c)
     cudaFree(c->scratch);
     cudaFree(c->gscratch);
     cudaFree(c->stage);
+    cudaFree(c->mc);
     for (int i = 0; i <= COS_MAX_ORDER; ++i) cudaFree(c->team_tabs[i]);
     if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
     for (cudaEvent_t e : c->copy_done) if (e) cudaEventDestroy(e);
@@ -424,6 +427,58 @@ int cos_debug_force_generic(cos_ctx* c, int enable)
 {
     if (!c) return COS_EINVAL;
     c->force_generic = enable != 0;
+    return COS_OK;
+}
+
+int cos_mc_run(cos_ctx* c, int n, long long walkers, int steps, unsigned long long seed, int* d_xy, double* d_tau,
+               double g_diag, double U, double* d_weight, unsigned char* d_accept_hist, long long* d_accepted,
+               double* d_sign_sum)
+{
+    if (!c || n < 1 || n > COS_MAX_ORDER || walkers < 0 || steps < 0) return COS_EINVAL;
+    if (walkers > 0 && (!d_xy || !d_tau || !d_weight)) return COS_EINVAL;
+    if (!c->table[0]) return COS_ENOTABLE;
+    if (c->table[1] && c->table[1] != c->table[0]) return COS_EINVAL;     // one table for both species (reading R19)
+    cudaSetDevice(c->device);
+    c->last_launches = 0;
+    if (walkers == 0) return COS_OK;
+    const size_t b_xy = (size_t)walkers * n * 2 * sizeof(int), b_tau = (size_t)walkers * n * sizeof(double);
+    const size_t b_w = (size_t)walkers * sizeof(double);
+    int rc = grow(c, &c->mc, &c->mc_bytes, b_tau + 2 * b_w + b_xy);
+    if (rc != COS_OK) return rc;
+    char* base = (char*)c->mc;
+    double* tau_p = (double*)base;
+    double* w_new = (double*)(base + b_tau);
+    double* w_alt = (double*)(base + b_tau + b_w);
+    int* xy_p = (int*)(base + b_tau + 2 * b_w);
+    if (d_accepted) COS_CUDA(c, cudaMemsetAsync(d_accepted, 0, (size_t)walkers * sizeof(long long), c->stream));
+    if (d_sign_sum) COS_CUDA(c, cudaMemsetAsync(d_sign_sum, 0, b_w, c->stream));
+    int launches = 0;
+    // weight of the initial configurations; the weight of the current state then alternates between two buffers so
+    // that the accept kernel never overwrites a value another thread of the same walker still has to read
+    double* w_cur = (steps % 2 == 0) ? d_weight : w_alt;
+    double* w_nxt = (steps % 2 == 0) ? w_alt : d_weight;
+    rc = cos_eval_connected_xt(c, n, walkers, d_xy, d_tau, g_diag, nullptr, U, w_cur);
+    if (rc != COS_OK) return rc;
+    launches += c->last_launches;
+    McArgs a{};
+    a.n = n; a.walkers = walkers; a.seed = seed; a.Lx = c->Lx; a.Ly = c->Ly; a.beta = c->beta;
+    a.xy = d_xy; a.tau = d_tau; a.xy_p = xy_p; a.tau_p = tau_p; a.w_new = w_new;
+    a.hist = d_accept_hist; a.accepted = d_accepted; a.sign_sum = d_sign_sum;
+    long long blocks = (walkers * n + 255) / 256;
+    const long long cap = (long long)c->num_sms * 16;
+    if (blocks > cap) blocks = cap;
+    for (int step = 0; step < steps; ++step) {
+        a.step = step; a.w_old = w_cur; a.w_out = w_nxt;
+        mc_propose_kernel<<<(unsigned)blocks, 256, 0, c->stream>>>(a);
+        COS_CUDA(c, cudaGetLastError());
+        rc = cos_eval_connected_xt(c, n, walkers, xy_p, tau_p, g_diag, nullptr, U, w_new);
+        if (rc != COS_OK) return rc;
+        launches += c->last_launches + 2;
+        mc_accept_kernel<<<(unsigned)blocks, 256, 0, c->stream>>>(a);
+        COS_CUDA(c, cudaGetLastError());
+        double* tmp = w_cur; w_cur = w_nxt; w_nxt = tmp;
+    }
+    c->last_launches = launches;      // after the last swap w_cur == d_weight
     return COS_OK;
 }
 
