@@ -107,6 +107,23 @@ int cos_eval_connected_xt_host(cos_ctx* ctx, int n, long long batch, const int* 
                                const double* h_tau, double g_diag, const double* h_u, double U,
                                double* h_out);
 
+/* FP32 variant of steps a2..a5.  The paper runs its graph in single precision throughout
+ * (Fig. 5 "FP32"; line 123: "the single-precision float value against double-precision ... on the
+ * order of 10^-5 % error ... order 10 configuration"; line 125: an uplift of up to 80 % against FP64).  Same arguments,
+ * layouts and return codes as cos_eval_all / cos_eval_connected (FP64 device arrays in and out): the library scales
+ * the matrices of every configuration by a power of two that brings their root-mean-square entry to [1, 2) (exact;
+ * the result is homogeneous of degree 2n in G, so it is multiplied by the inverse power on output -- without this
+ * the products of ten small Green's functions leave the FP32 range), rounds G and u once to FP32 into buffers of its
+ * own, and every later operation -- propagation, combine, connected reduction -- is FP32; the result is widened to
+ * FP64 on output.  Built for orders 1..10
+ * (COS_EINVAL above).  NOTE (reading R5): this build obtains `connected` by subtracting disconnected
+ * parts, so its FP32 error is about eps_32 * |D| / |C| per configuration, larger than the paper's figure, which is
+ * for a subtraction-free graph; DESIGN.md reports the measured distribution. */
+int cos_eval_all_f32(cos_ctx* ctx, int n, long long batch, const double* d_Gup, const double* d_Gdn,
+                     const double* d_u, double U, double* d_out);
+int cos_eval_connected_f32(cos_ctx* ctx, int n, long long batch, const double* d_Gup, const double* d_Gdn,
+                           const double* d_u, double U, double* d_out);
+
 /* On-device Monte Carlo over the vertex coordinates (reading R19).
  * (section II.B): "The integration over the vertex coordinates can then be performed by stochastic (Monte Carlo)
  * sampling"; line 137 (section IV.A): "one needs to handle proposal and acceptance of configurations ... readily

@@ -35,6 +35,8 @@ SIGNATURES = {
     "cos_build_G": (_int, [_vp, _int, _ll, _vp, _vp, _dbl, _vp, _vp]),
     "cos_eval_all": (_int, [_vp, _int, _ll, _vp, _vp, _vp, _dbl, _vp]),
     "cos_eval_connected": (_int, [_vp, _int, _ll, _vp, _vp, _vp, _dbl, _vp]),
+    "cos_eval_all_f32": (_int, [_vp, _int, _ll, _vp, _vp, _vp, _dbl, _vp]),
+    "cos_eval_connected_f32": (_int, [_vp, _int, _ll, _vp, _vp, _vp, _dbl, _vp]),
     "cos_eval_connected_xt": (_int, [_vp, _int, _ll, _vp, _vp, _dbl, _vp, _dbl, _vp]),
     "cos_eval_connected_xt_host": (_int, [_vp, _int, _ll, _vp, _vp, _dbl, _vp, _dbl, _vp]),
     "cos_mc_run": (_int, [_vp, _int, _ll, _int, ctypes.c_ulonglong, _vp, _vp, _dbl, _dbl, _vp, _vp, _vp, _vp]),
@@ -215,6 +217,15 @@ class Context:
     def eval_connected(self, d_Gup, d_Gdn, d_out, U: float = 1.0, d_u=None):
         n, batch, gu, gd, u, out = self._eval_ptrs(d_Gup, d_Gdn, d_out, d_u)
         self._check(self._lib.cos_eval_connected(self._h, n, batch, gu, gd, u, float(U), out))
+
+    def eval_all_f32(self, d_Gup, d_Gdn, d_out, U: float = 1.0, d_u=None):
+        """FP32 variant (include/cos.h: cos_eval_all_f32); FP64 tensors in and out."""
+        n, batch, gu, gd, u, out = self._eval_ptrs(d_Gup, d_Gdn, d_out, d_u)
+        self._check(self._lib.cos_eval_all_f32(self._h, n, batch, gu, gd, u, float(U), out))
+
+    def eval_connected_f32(self, d_Gup, d_Gdn, d_out, U: float = 1.0, d_u=None):
+        n, batch, gu, gd, u, out = self._eval_ptrs(d_Gup, d_Gdn, d_out, d_u)
+        self._check(self._lib.cos_eval_connected_f32(self._h, n, batch, gu, gd, u, float(U), out))
 
     def eval_connected_xt(self, d_xy, d_tau, d_out, U: float = 1.0, d_u=None, g_diag: float = 0.0):
         batch, n = (int(s) for s in d_tau.shape)

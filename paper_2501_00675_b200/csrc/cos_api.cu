@@ -9,7 +9,6 @@
 
 #include "cos_common.cuh"
 #include "cos_internal.h"
-#include "cos_kernels_generic.cuh"
 #include "cos_dispatch.cuh"
 #include "cos_mc.cuh"
 
@@ -31,6 +30,8 @@ struct cos_ctx {
     unsigned char* team_tabs[COS_MAX_ORDER + 1] = {};            // per order: table image of the team kernel / item
                                                                  // descriptors of the pair kernel
     void* stage = nullptr;          size_t stage_bytes = 0;      // device staging of the host path
+    unsigned char* team_tabs32[COS_MAX_ORDER + 1] = {};          // FP32 variant: table images of the team kernel
+    float* g32 = nullptr;           size_t g32_bytes = 0;        // FP32 variant: converted copies of G_up, G_down, u
     void* mc = nullptr;             size_t mc_bytes = 0;         // cos_mc_run: proposal coordinates and weights
     cudaStream_t copy_stream = nullptr;                          // host path: H2D of chunk k+1 behind the kernels of chunk k
     cudaEvent_t copy_done[2] = {nullptr, nullptr};
@@ -133,10 +134,10 @@ int do_eval(cos_ctx* c, int n, long long batch, const double* gup, const double*
         // no tables: the generic kernel computes its indices on the fly
     } else if (uses_team(n)) {   // table image of this order, built on first use
         if (!c->team_tabs[n]) {
-            const TeamDims td = team_choice(n, 1).d;
+            const f64::TeamDims td = team_choice(n, 1).d;
             unsigned char* buf = nullptr;
             if (alloc_dev(c, (void**)&buf, (size_t)td.tab_bytes) != COS_OK) return COS_ENOMEM;
-            team_tables_kernel<<<1, 256, (size_t)td.tab_bytes, c->stream>>>(td, buf);
+            f64::team_tables_kernel<<<1, 256, (size_t)td.tab_bytes, c->stream>>>(td, buf);
             COS_CUDA(c, cudaGetLastError());
             c->team_tabs[n] = buf;
         }
@@ -162,6 +163,93 @@ int do_eval(cos_ctx* c, int n, long long batch, const double* gup, const double*
         a.scratch_stride = per_cta;
     }
     return launch_eval(c, a);
+}
+
+// FP32 variant, input side: one warp per configuration.  Every term of the result is homogeneous of degree 2n in
+// the entries of G (n factors per species), so G is first scaled by a power of two s = 2^k (exact) that brings
+// its root-mean-square entry to [1, 2): products of ten small Green's functions would otherwise leave the FP32
+// range (cfg3: Z ~ 1e-20, D ~ Z^2 underflows).  The output kernel multiplies the result by 2^(-2nk).
+__global__ void __launch_bounds__(256) convert_scale_f32_kernel(int n, long long batch, const double* __restrict__ gup,
+                                                                const double* __restrict__ gdn, float* __restrict__ gu32,
+                                                                float* __restrict__ gd32, int* __restrict__ kexp)
+{
+    const int lane = threadIdx.x & 31, nn = n * n;
+    for (long long b = (blockIdx.x * (long long)blockDim.x + threadIdx.x) >> 5; b < batch;
+         b += ((long long)gridDim.x * blockDim.x) >> 5) {
+        const double* pu = gup + b * nn;
+        const double* pd = gdn + b * nn;
+        double ss = 0.0;
+        for (int e = lane; e < nn; e += 32) { const double x = pu[e], y = pd[e]; ss += x * x + y * y; }
+        for (int o = 16; o > 0; o >>= 1) ss += __shfl_xor_sync(0xffffffffu, ss, o);
+        int k = 0;
+        if (ss > 0.0 && ss - ss == 0.0) k = -ilogb(sqrt(ss / (2.0 * nn)));      // rms * 2^k in [1, 2)
+        const double sc = ldexp(1.0, k);
+        for (int e = lane; e < nn; e += 32) {
+            gu32[b * nn + e] = (float)(pu[e] * sc);                              // one rounding, to nearest even
+            if (gd32 != gu32) gd32[b * nn + e] = (float)(pd[e] * sc);
+        }
+        if (lane == 0) kexp[b] = k;
+    }
+}
+
+__global__ void __launch_bounds__(256) convert_f64_f32_kernel(const double* __restrict__ src, float* __restrict__ dst, size_t count)
+{
+    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < count; i += (size_t)gridDim.x * blockDim.x)
+        dst[i] = (float)src[i];                       // round to nearest even
+}
+
+__global__ void __launch_bounds__(256) unscale_f32_kernel(int n, long long batch, const int* __restrict__ kexp, double* out)
+{
+    for (long long b = blockIdx.x * (long long)blockDim.x + threadIdx.x; b < batch; b += (long long)gridDim.x * blockDim.x)
+        out[b] = ldexp(out[b], -2 * n * kexp[b]);
+}
+
+// FP32 variant: G and u are rounded once to FP32, every later operation is FP32.
+int do_eval_f32(cos_ctx* c, int n, long long batch, const double* gup, const double* gdn, const double* u, double U,
+                double* out, int connected)
+{
+    if (n > kF32MaxN) return COS_EINVAL;
+    if (batch == 0) return COS_OK;
+    const bool two = gdn != gup;
+    const size_t nn = (size_t)batch * n * n, nu = u ? (size_t)batch * n : 0;
+    int rc = grow(c, (void**)&c->g32, &c->g32_bytes, sizeof(float) * ((two ? 2 : 1) * nn + nu) + sizeof(int) * (size_t)batch);
+    if (rc != COS_OK) return rc;
+    float* gu32 = c->g32;
+    float* gd32 = two ? gu32 + nn : gu32;
+    float* u32 = u ? gu32 + (two ? 2 : 1) * nn : nullptr;
+    int* kexp = reinterpret_cast<int*>(gu32 + (two ? 2 : 1) * nn + nu);
+    const unsigned blocks = (unsigned)c->num_sms * 8;
+    convert_scale_f32_kernel<<<blocks, 256, 0, c->stream>>>(n, batch, gup, gdn, gu32, gd32, kexp);
+    if (u) convert_f64_f32_kernel<<<blocks, 256, 0, c->stream>>>(u, u32, nu);
+    COS_CUDA(c, cudaGetLastError());
+    c->last_launches += 2 + (u ? 1 : 0);
+    EvalArgs a{};
+    a.n = n; a.batch = batch; a.U = U; a.out = out; a.connected = connected; a.off = c->off; a.loopf = -c->loop_weight;
+    a.Gup = reinterpret_cast<const double*>(gu32);      // FP32 data behind the FP64-typed fields (read through in_real)
+    a.Gdn = reinterpret_cast<const double*>(gd32);
+    a.u = reinterpret_cast<const double*>(u32);
+    if (uses_team(n)) {
+        if (!c->team_tabs32[n]) {
+            const f32::TeamDims td = team_choice_f32(n, 1).d;
+            unsigned char* buf = nullptr;
+            if (alloc_dev(c, (void**)&buf, (size_t)td.tab_bytes) != COS_OK) return COS_ENOMEM;
+            f32::team_tables_kernel<<<1, 256, (size_t)td.tab_bytes, c->stream>>>(td, buf);
+            COS_CUDA(c, cudaGetLastError());
+            c->team_tabs32[n] = buf;
+        }
+        a.tabs = c->team_tabs32[n];
+    }
+    const bool t = timer_begin(c);
+    int launches = 0;
+    const char* name = nullptr;
+    cudaError_t e = dispatch_eval_f32(a, c->stream, c->num_sms, &launches, &name);
+    if (t) timer_end(c);
+    if (e != cudaSuccess) return fail_cuda(c, e);
+    unscale_f32_kernel<<<blocks, 256, 0, c->stream>>>(n, batch, kexp, out);
+    COS_CUDA(c, cudaGetLastError());
+    c->last_launches += launches;
+    c->last_kernel = name;
+    return COS_OK;
 }
 
 int do_build_G(cos_ctx* c, int n, long long batch, const int* xy, const double* tau, double g_diag,
@@ -258,6 +346,8 @@ int cos_destroy(cos_ctx* c)
     cudaFree(c->gscratch);
     cudaFree(c->stage);
     cudaFree(c->mc);
+    cudaFree(c->g32);
+    for (int i = 0; i <= COS_MAX_ORDER; ++i) cudaFree(c->team_tabs32[i]);
     for (int i = 0; i <= COS_MAX_ORDER; ++i) cudaFree(c->team_tabs[i]);
     if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
     for (cudaEvent_t e : c->copy_done) if (e) cudaEventDestroy(e);
@@ -308,6 +398,26 @@ int cos_eval_connected(cos_ctx* c, int n, long long batch, const double* d_Gup, 
     cudaSetDevice(c->device);
     c->last_launches = 0;
     return do_eval(c, n, batch, d_Gup, d_Gdn, d_u, U, d_out, 1);
+}
+
+int cos_eval_all_f32(cos_ctx* c, int n, long long batch, const double* d_Gup, const double* d_Gdn,
+                     const double* d_u, double U, double* d_out)
+{
+    int rc = check_eval_args(c, n, batch, d_Gup, d_Gdn, d_out);
+    if (rc != COS_OK) return rc;
+    cudaSetDevice(c->device);
+    c->last_launches = 0;
+    return do_eval_f32(c, n, batch, d_Gup, d_Gdn, d_u, U, d_out, 0);
+}
+
+int cos_eval_connected_f32(cos_ctx* c, int n, long long batch, const double* d_Gup, const double* d_Gdn,
+                           const double* d_u, double U, double* d_out)
+{
+    int rc = check_eval_args(c, n, batch, d_Gup, d_Gdn, d_out);
+    if (rc != COS_OK) return rc;
+    cudaSetDevice(c->device);
+    c->last_launches = 0;
+    return do_eval_f32(c, n, batch, d_Gup, d_Gdn, d_u, U, d_out, 1);
 }
 
 int cos_eval_halfvertex(cos_ctx* c, int n_lines, long long batch, const double* d_W, const double* d_V, int connected,

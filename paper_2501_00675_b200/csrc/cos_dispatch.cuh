@@ -9,16 +9,16 @@
 #pragma once
 #include "cos_common.cuh"
 #include "cos_kernels_generic.cuh"
-#include "cos_kernels_team.cuh"
+#include "cos_kernels_typed.cuh"
 #include "cos_kernels_pair.cuh"
 
 namespace cosb {
 
 constexpr int kGenericThreads = 256;
 
-inline size_t generic_smem_bytes(int n, int nsp)
+inline size_t generic_smem_bytes(int n, int nsp, size_t elem = sizeof(double))
 {
-    return sizeof(double) * (generic_small_doubles(n) + ((size_t)nsp << n) + generic_frontier_doubles(n));
+    return elem * (generic_small_doubles(n) + ((size_t)nsp << n) + generic_frontier_doubles(n));
 }
 
 // True when the generic kernel must keep Z and the frontier in global scratch.
@@ -34,16 +34,28 @@ inline size_t generic_scratch_doubles(int n, int smem_optin)
 
 // ---- team kernel (orders 5..10): instances per team and launch shape per order ----
 constexpr int kTeamMinN = 5, kTeamMaxN = 10;
-using TeamKernel = void (*)(EvalArgs, TeamDims);
-struct TeamChoice { TeamKernel fn; TeamDims d; };
+using TeamKernel = void (*)(EvalArgs, f64::TeamDims);
+struct TeamChoice { TeamKernel fn; f64::TeamDims d; };
 inline bool uses_team(int n) { return n >= kTeamMinN && n <= kTeamMaxN; }
 inline TeamChoice team_choice(int n, int nsp)
 {
-    if (n == 10) return {eval_team_kernel<4, 160, 2>, team_dims<4>(n, nsp)};
-    if (n == 9) return {eval_team_kernel<8, 160, 2>, team_dims<8>(n, nsp)};
-    if (n == 8) return {eval_team_kernel<16, 160, 2>, team_dims<16>(n, nsp)};
-    return {eval_team_kernel<32, 192, 2>, team_dims<32>(n, nsp)};
+    if (n == 10) return {f64::eval_team_kernel<4, 160, 2>, f64::team_dims<4>(n, nsp)};
+    if (n == 9) return {f64::eval_team_kernel<8, 160, 2>, f64::team_dims<8>(n, nsp)};
+    if (n == 8) return {f64::eval_team_kernel<16, 160, 2>, f64::team_dims<16>(n, nsp)};
+    return {f64::eval_team_kernel<32, 192, 2>, f64::team_dims<32>(n, nsp)};
 }
+// FP32 variant: the same kernels instantiated for float; half the shared memory per instance, so
+// more teams are resident per SM (the launch bounds only cap the registers)
+using TeamKernel32 = void (*)(EvalArgs, f32::TeamDims);
+struct TeamChoice32 { TeamKernel32 fn; f32::TeamDims d; };
+inline TeamChoice32 team_choice_f32(int n, int nsp)
+{
+    if (n == 10) return {f32::eval_team_kernel<4, 160, 3>, f32::team_dims<4>(n, nsp)};
+    if (n == 9) return {f32::eval_team_kernel<8, 160, 3>, f32::team_dims<8>(n, nsp)};
+    if (n == 8) return {f32::eval_team_kernel<16, 160, 3>, f32::team_dims<16>(n, nsp)};
+    return {f32::eval_team_kernel<32, 192, 2>, f32::team_dims<32>(n, nsp)};
+}
+constexpr int kF32MaxN = kTeamMaxN;       // the FP32 variant is built for orders 1..10 (generic + team kernels)
 
 // ---- pair kernel (orders 11..13): the team mapping with every item split over a lane pair ----
 constexpr int kPairMinN = 11, kPairMaxN = 13;
@@ -90,11 +102,15 @@ inline int eval_max_ctas(long long batch, int num_sms)
 
 inline cudaError_t configure_kernels(int smem_optin)
 {
-    cudaError_t e = cudaFuncSetAttribute(eval_generic_kernel<kGenericThreads>,
+    cudaError_t e = cudaFuncSetAttribute(f64::eval_generic_kernel<kGenericThreads>,
                                          cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
+    if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(f32::eval_generic_kernel<kGenericThreads>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
     if (e != cudaSuccess) return e;
     for (int n = kTeamMinN; n <= kTeamMaxN; ++n) {
         e = cudaFuncSetAttribute(team_choice(n, 1).fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
+        if (e != cudaSuccess) return e;
+        e = cudaFuncSetAttribute(team_choice_f32(n, 1).fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
         if (e != cudaSuccess) return e;
     }
     for (int n = kPairMinN; n <= kPairMaxN; ++n) {
@@ -146,7 +162,7 @@ inline cudaError_t dispatch_eval(const EvalArgs& a, cudaStream_t stream, int num
     if (use_global && a.scratch == nullptr) return cudaErrorInvalidValue;
     const size_t smem = use_global ? sizeof(double) * generic_small_doubles(a.n) : generic_smem_bytes(a.n, nsp);
     int per_sm = 1;
-    cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, eval_generic_kernel<kGenericThreads>,
+    cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, f64::eval_generic_kernel<kGenericThreads>,
                                                                   kGenericThreads, smem);
     if (e != cudaSuccess) return e;
     if (per_sm < 1) per_sm = 1;
@@ -156,8 +172,33 @@ inline cudaError_t dispatch_eval(const EvalArgs& a, cudaStream_t stream, int num
         if (grid > cap) grid = cap;
     }
     if (grid > a.batch) grid = a.batch;
-    eval_generic_kernel<kGenericThreads><<<(unsigned)grid, kGenericThreads, smem, stream>>>(a, nsp, use_global ? 1 : 0);
+    f64::eval_generic_kernel<kGenericThreads><<<(unsigned)grid, kGenericThreads, smem, stream>>>(a, nsp, use_global ? 1 : 0);
     *name = "eval_generic_kernel";
+    return cudaGetLastError();
+}
+
+// FP32 variant: orders 1..4 on the plain kernel, 5..10 on the team kernel, both instantiated for float.  The input
+// pointers of `a` address FP32 copies of G and u (made by the entry point).
+inline cudaError_t dispatch_eval_f32(const EvalArgs& a, cudaStream_t stream, int num_sms, int* launches, const char** name)
+{
+    const int nsp = (a.Gdn == a.Gup) ? 1 : 2;
+    *launches = 1;
+    if (uses_team(a.n)) {
+        const TeamChoice32 tc = team_choice_f32(a.n, nsp);
+        *name = "eval_team_kernel<float>";
+        return launch_persistent(tc.fn, tc.d, a, (a.batch * nsp + tc.d.C - 1) / tc.d.C, 0, num_sms, stream);
+    }
+    if (a.n > kF32MaxN) return cudaErrorInvalidValue;
+    const size_t smem = generic_smem_bytes(a.n, nsp, sizeof(float));
+    int per_sm = 1;
+    cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, f32::eval_generic_kernel<kGenericThreads>,
+                                                                  kGenericThreads, smem);
+    if (e != cudaSuccess) return e;
+    if (per_sm < 1) per_sm = 1;
+    long long grid = (long long)num_sms * per_sm;
+    if (grid > a.batch) grid = a.batch;
+    f32::eval_generic_kernel<kGenericThreads><<<(unsigned)grid, kGenericThreads, smem, stream>>>(a, nsp, 0);
+    *name = "eval_generic_kernel<float>";
     return cudaGetLastError();
 }
 

@@ -103,155 +103,4 @@ __host__ __device__ inline size_t generic_frontier_doubles(int n)
 }
 __host__ __device__ inline size_t generic_small_doubles(int n) { return (size_t)2 * n * n + 16; }
 
-template <int kThreads>
-__global__ void __launch_bounds__(kThreads) eval_generic_kernel(EvalArgs a, int nsp, int use_global)
-{
-    extern __shared__ double smem[];
-    const int n = a.n;
-    const int tid = threadIdx.x;
-    const unsigned N = 1u << n;
-    double* W = smem;                       // [nsp][n][n]
-    double* uvec = smem + 2 * n * n;        // [n] (-u_a)
-    double* Z;                              // [nsp][N]
-    double* P;                              // frontier of the current stage / C' in the reduction
-    if (use_global) {
-        Z = a.scratch + (size_t)blockIdx.x * a.scratch_stride;
-        P = Z + (size_t)2 * N;
-    } else {
-        Z = smem + generic_small_doubles(n);
-        P = Z + (size_t)nsp * N;
-    }
-    const uint32_t* __restrict__ off = a.off;
-
-    for (long long b = blockIdx.x; b < a.batch; b += gridDim.x) {
-        __syncthreads();
-        // ---- load W (both species) and the couplings; fold -u_a into the rows of W_up when the
-        //      species are distinct (each term has exactly one factor from every row of S) ----
-        const int nu = a.halfvertex ? n / 2 : n;             // couplings: per vertex, or per interaction line (R18)
-        for (int t = tid; t < nu; t += kThreads) uvec[t] = -(a.u ? a.u[b * nu + t] : a.U);
-        __syncthreads();
-        for (int t = tid; t < n * n; t += kThreads) {
-            const double g = a.Gup[b * n * n + t];
-            W[t] = (nsp == 2) ? g * uvec[t / n] : g;
-            if (nsp == 2) W[n * n + t] = a.Gdn[b * n * n + t];
-        }
-        __syncthreads();
-
-        // ---- a2: propagation, one species after the other ----
-        for (int s = 0; s < nsp; ++s) {
-            const double* Ws = W + s * n * n;
-            double* Zs = Z + (size_t)s * N;
-            if (tid == 0) Zs[0] = 1.0;                      // top node = 1
-            __syncthreads();
-            for (int h = 0; h < n; ++h) {
-                const unsigned NR = 1u << h;
-                for (unsigned R = tid; R < NR; R += kThreads)   // start: P_h[R][h] = Z[R]
-                    P[off[R] + __popc(R)] = Zs[R];
-                __syncthreads();
-                for (int j = 0; j <= h; ++j) {
-                    for (unsigned R = tid; R < NR; R += kThreads) {
-                        if (__popc(R) != j) continue;
-                        const double* pr = P + off[R];
-                        const double ah = pr[j];
-                        // close: Z[R + {h}] = - sum_c P[R][c] W[c][h]
-                        {
-                            double acc = ah * Ws[h * n + h];
-                            unsigned m = R; int i = 0;
-                            while (m) { const int c = __ffs(m) - 1; m &= m - 1; acc = fma(pr[i++], Ws[c * n + h], acc); }
-                            Zs[R | NR] = a.loopf * acc;            // -1 per closed fermion loop, -N_f in general (R17)
-                        }
-                        // extend to every c' < h not in R
-                        unsigned absent = ~R & (NR - 1);
-                        while (absent) {
-                            const int cp = __ffs(absent) - 1; absent &= absent - 1;
-                            double acc = ah * Ws[h * n + cp];
-                            unsigned m = R; int i = 0;
-                            while (m) { const int c = __ffs(m) - 1; m &= m - 1; acc = fma(pr[i++], Ws[c * n + cp], acc); }
-                            const unsigned R2 = R | (1u << cp);
-                            P[off[R2] + __popc(R2 & ((1u << cp) - 1))] = acc;
-                        }
-                    }
-                    __syncthreads();
-                }
-            }
-        }
-
-        const double* Zup = Z;
-        const double* Zdn = Z + (size_t)(nsp - 1) * N;
-        if (!a.connected) {                                  // a5 "all": D[full]
-            if (tid == 0) {
-                double w = 1.0;
-                if (nsp == 1) for (int v = 0; v < nu; ++v) w *= uvec[v];
-                a.out[b] = w * Zup[N - 1] * (a.halfvertex ? 1.0 : Zdn[N - 1]);
-            }
-            continue;
-        }
-
-        // ---- a3: D[S] = w(S) Zup[S] Zdn[S], stored over Zup.  Half-vertex formulation (R18): the reduction runs
-        //      over the n' interaction lines, D'[P] = prod_{k in P}(-V_k) Z[both half-vertices of every line of P],
-        //      stored in the (now free) frontier area ----
-        int nr = n;                                          // bits of the reduction
-        double* D = Z;
-        double* C = P;
-        if (a.halfvertex) {
-            nr = n / 2;
-            D = P;
-            C = P + ((size_t)1 << nr);
-            for (unsigned Pm = tid; Pm < (1u << nr); Pm += kThreads) {
-                double w = 1.0;
-                unsigned S = 0, m = Pm;
-                while (m) { const int k = __ffs(m) - 1; m &= m - 1; w *= uvec[k]; S |= 3u << (2 * k); }
-                D[Pm] = w * Zup[S];
-            }
-        } else {
-            for (unsigned S = tid; S < N; S += kThreads) {
-                double w = 1.0;
-                if (nsp == 1) { unsigned m = S; while (m) { const int v = __ffs(m) - 1; m &= m - 1; w *= uvec[v]; } }
-                D[S] = w * Zup[S] * Zdn[S];
-            }
-        }
-        __syncthreads();
-
-        // ---- a4: C'[S'] = D[2S'+1] - sum_{T' proper subset of S'} C'[T'] D[2(S'\T')], levels |S'| ----
-        const unsigned M = 1u << (nr - 1);                   // subsets of vertices (lines) 1..nr-1
-        const int lane = tid & 31, warp = tid >> 5, nwarps = kThreads >> 5;
-        for (int l = 0; l < nr; ++l) {
-            if (l < 5) {
-                for (unsigned Sp = tid; Sp < M; Sp += kThreads) {
-                    if (__popc(Sp) != l) continue;
-                    double acc = D[2 * Sp + 1];
-                    for (unsigned Tp = (Sp - 1) & Sp; Sp != 0; Tp = (Tp - 1) & Sp) {
-                        acc = fma(-C[Tp], D[2 * (Sp ^ Tp)], acc);
-                        if (Tp == 0) break;
-                    }
-                    C[Sp] = acc;
-                }
-            } else {
-                // one warp per output; lanes own the 32 sub-subsets of the 5 lowest vertices of S'
-                for (unsigned Sp = warp; Sp < M; Sp += nwarps) {
-                    if (__popc(Sp) != l) continue;
-                    unsigned low5 = 0, tlo = 0, m = Sp;
-                    for (int q = 0; q < 5; ++q) {
-                        const unsigned bit = m & (0u - m); m ^= bit; low5 |= bit;
-                        if (lane >> q & 1) tlo |= bit;
-                    }
-                    const unsigned Shi = Sp ^ low5;
-                    double acc = 0.0;
-                    unsigned Thi = Shi;
-                    while (true) {
-                        const unsigned Tp = Thi | tlo;
-                        if (Tp != Sp) acc = fma(C[Tp], D[2 * (Sp ^ Tp)], acc);
-                        if (Thi == 0) break;
-                        Thi = (Thi - 1) & Shi;
-                    }
-                    for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
-                    if (lane == 0) C[Sp] = D[2 * Sp + 1] - acc;
-                }
-            }
-            __syncthreads();
-        }
-        if (tid == 0) a.out[b] = C[M - 1];
-    }
-}
-
 }  // namespace cosb

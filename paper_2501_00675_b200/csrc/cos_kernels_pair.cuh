@@ -24,10 +24,10 @@
 //   W entry (c, c') of instance g, replica r:                (c * n + c') * 16 + r * C + g     (16 / C replicas)
 #pragma once
 #include "cos_common.cuh"
-#include "cos_kernels_generic.cuh"
-#include "cos_kernels_team.cuh"    // RedLayout, team_reduce (connected reduction on interleaved blocks)
+#include "cos_kernels_typed.cuh"   // f64::RedLayout, f64::team_reduce (connected reduction on interleaved blocks)
 
 namespace cosb {
+using namespace f64;
 
 constexpr int kPairB = 3;            // |T|
 constexpr int kPairMaxCols = 9;      // Q-targets + close held in registers (order 12: at most 8 + 1)
