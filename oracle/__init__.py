@@ -17,7 +17,11 @@ import subprocess
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_SO = os.path.join(_HERE, "liboracle.so")
+# COS_ORACLE_SANITIZE=1: a second build with AddressSanitizer + UndefinedBehaviorSanitizer, used as
+#   COS_ORACLE_SANITIZE=1 LD_PRELOAD=$(gcc -print-file-name=libasan.so) ASAN_OPTIONS=detect_leaks=0 \
+#       python -m pytest tests -m "not gpu" -k oracle
+_SANITIZE = os.environ.get("COS_ORACLE_SANITIZE", "") not in ("", "0")
+_SO = os.path.join(_HERE, "liboracle_san.so" if _SANITIZE else "liboracle.so")
 _SRC = [os.path.join(_HERE, "cos_oracle.c"), os.path.join(_HERE, "cos_oracle_core.inc")]
 _lib = None
 
@@ -32,6 +36,8 @@ def build(force: bool = False) -> str:
     if stale:
         cmd = ["gcc", "-O2", "-std=c11", "-ffp-contract=off", "-fopenmp", "-shared", "-fPIC",
                _SRC[0], "-o", _SO, "-lm"]
+        if _SANITIZE:
+            cmd[1:1] = ["-g", "-fsanitize=address,undefined", "-fno-sanitize-recover=undefined", "-fno-omit-frame-pointer"]
         subprocess.run(cmd, check=True, cwd=_HERE)
     return _SO
 

@@ -343,3 +343,29 @@ def test_halfvertex(torch_mod, oracle_mod, nl):
                 bad = np.abs(got - ref) > 1e-10 * np.abs(ref)
                 assert bad.sum() <= max(1, int(np.ceil(2e-3 * B))), (nl, nf, connected, np.abs(got / ref - 1).max())
                 assert np.all(np.abs(got - ref) <= 1e-7 * np.abs(ref))
+
+
+# ------------------------------------------------------------------------------------------ races / stale state
+@pytest.mark.parametrize("n,nsp", [(3, 1), (6, 2), (8, 1), (9, 2), (10, 1), (10, 2), (11, 1), (12, 2), (13, 1), (13, 2),
+                                   (14, 1), (15, 1)])
+def test_result_independent_of_batch_position_and_repeatable(torch_mod, ctx, n, nsp):
+    """compute-sanitizer is closed on this GPU pool, so data races and stale shared-memory / scratch state are hunted
+    with properties they would break: (1) the value of a configuration does not depend on where it sits in the batch
+    (other team mates, another lane group, another W replica, another persistent CTA, first or last team of the
+    loop) -- bit for bit; (2) repeated launches give identical bits.  Batches give every persistent CTA several teams."""
+    torch = torch_mod
+    rng = np.random.default_rng(8000 + 10 * n + nsp)
+    B = _MANY[n] // (2 if n >= 13 else 1)
+    Gup = rng.normal(size=(B, n, n)) / np.sqrt(n) + 0.5 * np.eye(n)
+    Gdn = rng.normal(size=(B, n, n)) / np.sqrt(n) + 0.5 * np.eye(n) if nsp == 2 else None
+    u = rng.uniform(0.5, 2.0, size=(B, n))
+    perm = rng.permutation(B)
+    a = _gpu_eval(torch, ctx, Gup, Gdn, 1.0, u, "connected")
+    b = _gpu_eval(torch, ctx, Gup[perm], None if Gdn is None else Gdn[perm], 1.0, u[perm], "connected")
+    np.testing.assert_array_equal(a[perm], b)
+    for _ in range(3):
+        np.testing.assert_array_equal(_gpu_eval(torch, ctx, Gup, Gdn, 1.0, u, "connected"), a)
+    # a ragged sub-batch (different team boundaries, fewer CTAs) reproduces the same bits for the configurations it holds
+    k = max(1, B // 3 + 1)
+    c = _gpu_eval(torch, ctx, Gup[:k], None if Gdn is None else Gdn[:k], 1.0, u[:k], "connected")
+    np.testing.assert_array_equal(c, a[:k])

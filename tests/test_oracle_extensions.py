@@ -215,7 +215,7 @@ def test_abs_sum_is_the_majorant_of_the_recursion(oracle_mod, n):
     """What oracle_abs_sum(s) returns, written out: with |D|[S] = prod|u| perm|Gup[S,S]| perm|Gdn[S,S]| (Ryser),
     abs_all = |D|[full] and abs_conn = the sum of |every product the subset recursion forms| when it is unrolled,
     i.e. sum over T1 containing vertex 0 of |D|[T1] times the sum over ORDERED partitions (B1..Bk) of the remaining
-    vertices of prod |D|[Bi]  (each subtraction C[T] D[S \ T] of the recursion, expanded down to D's)."""
+    vertices of prod |D|[Bi]  (each subtraction C[T] D[S minus T] of the recursion, expanded down to D's)."""
     rng = np.random.default_rng(300 + n)
     Gup, Gdn, u = rng.normal(size=(n, n)), rng.normal(size=(n, n)), rng.uniform(0.5, 2.0, size=n)
 
