@@ -75,9 +75,17 @@ def get_workload(name: str, rank: int = 0):
 
 
 # ----------------------------------------------------------------------------------------------
-# dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel, per launch, from the committed ncu capture
-# (profiles/r1c_launches_default_bench.md, "DRAM traffic"); None for workloads that were not captured.
-NCU_TRAFFIC = {"cfg3_n10_b16384": 13198848 + 0}
+def ncu_traffic(workload_name: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel, per launch, parsed from the committed ncu
+    summary profiles/r2_traffic.json (written from one `ncu --set full` capture per workload; the file names the
+    command).  None when the workload was not captured -- nothing is measured under a profiler in this run."""
+    path = os.path.join(ROOT, "profiles", "r2_traffic.json")
+    try:
+        with open(path) as f:
+            rec = json.load(f).get(workload_name)
+        return None if rec is None else {"bytes": rec["dram_bytes"], "source": "profiles/r2_traffic.json: " + rec["capture"]}
+    except (OSError, ValueError, KeyError):
+        return None
 
 
 class ClockSampler:
@@ -201,7 +209,22 @@ def cpu_baseline(w, target_seconds: float = 12.0):
     dt = time.perf_counter() - t0
     return {"value": sample / dt, "unit": UNIT, "cores": int(cores), "kind": "oracle",
             "sample": f"first {sample} of {w.batch} configurations of {w.name} (G assembly + all/connected evaluation, "
-                      f"OpenMP over configurations, {dt:.2f} s)"}
+                      f"OpenMP over configurations, {dt:.2f} s)"}, sample
+
+
+def parity_on_sample(w, gpu_out, sample):
+    """The timed GPU outputs of the first `sample` configurations against the oracle (strict 1e-10 count; the
+    conditioning exceptions of DESIGN.md §4 are judged by tests/parity_util.py, here they are only counted)."""
+    import oracle
+    if w.kind == "hubbard":
+        g, _ = oracle.build_G(w.xy[:sample], w.tau[:sample], w.table, None, w.beta, w.g_diag)
+        u = None
+    else:
+        g, u = w.G[:sample], w.u[:sample]
+    _, ref = oracle.eval_all_connected(g, None, U=w.U, u=u)
+    rel = np.abs(gpu_out[:sample] - ref) / np.abs(ref)
+    return {"configurations": int(sample), "max_rel_err": float(rel.max()), "median_rel_err": float(np.median(rel)),
+            "over_1e-10": int((rel > 1e-10).sum())}
 
 
 # ----------------------------------------------------------------------------------------------
@@ -387,12 +410,19 @@ def run_ours(args):
                      "peak_source": "cos_probe_dfma: register-only FP64 FMA kernel measured in this run "
                                     "(MEASURED_PEAKS.json has no FP64 figure); nominal 148 SM x 64 FMA/clk x 1.965 GHz = 37.2",
                      "kernel_ms": kern_ms, "kernel_launches_timed": kern_launches,
-                     "smem_probe_gbs": smem_gbs, "traffic": NCU_TRAFFIC.get(w.name)},
+                     "smem_probe_gbs": smem_gbs, "traffic": None},
     }
+    tr = ncu_traffic(w.name)
+    if tr is not None:
+        line["roofline"]["traffic"] = tr["bytes"]
+        line["roofline"]["traffic_source"] = tr["source"]
     if not args.no_cpu_baseline and world == 1:
-        line["cpu_baseline"] = cpu_baseline(w)
+        line["cpu_baseline"], sample = cpu_baseline(w)
+        line["parity_sample"] = parity_on_sample(w, runner.out.cpu().numpy(), sample)
     if not args.no_sweep and world == 1:
         line["two_species"] = two_species_line(torch, api, runner, flush, dfma_tflops)
+        line["f32"] = f32_line(torch, api, runner, flush)
+        line["mc"] = mc_line(torch, runner, flush, kern_ms)
         line["sweep"] = sweep(torch, api, local_rank, flush, dfma_tflops)
     print(json.dumps(line))
     if world > 1:
@@ -454,6 +484,70 @@ def two_species_line(torch, api, runner, flush, dfma_tflops):
             "flop_per_config": flop, "kernel_tflops": flop * w.batch / (kern_ms * 1e-3) * 1e-12,
             "frac_of_dfma_peak": flop * w.batch / (kern_ms * 1e-3) * 1e-12 / dfma_tflops,
             "kernel": ctx.last_kernel_name(), "kernel_ms": kern_ms, "matches_one_species_result": same}
+
+
+def f32_line(torch, api, runner, flush):
+    """FP32 variant ("uplift of up to 80 %") on the headline workload: kernel time against
+    the FP64 kernel on the same matrices, and the FP32-vs-FP64 error of the results."""
+    w = runner.w
+    if w.kind != "hubbard" or w.n > 10:
+        return None
+    ctx = runner.ctx
+    G = torch.empty((w.batch, w.n, w.n), dtype=torch.float64, device="cuda")
+    ctx.build_G(runner.xy, runner.tau, G, None, g_diag=w.g_diag)
+    o64 = torch.empty(w.batch, dtype=torch.float64, device="cuda")
+    o32 = torch.empty_like(o64)
+    ms = {}
+    ctx.enable_kernel_timer(True)
+    for name, fn, out in (("f64", ctx.eval_connected, o64), ("f32", ctx.eval_connected_f32, o32)):
+        for _ in range(3):
+            fn(G, G, out, U=w.U)
+        torch.cuda.synchronize()
+        ctx.reset_kernel_timer()
+        for _ in range(5):
+            flush.fill_(1)
+            fn(G, G, out, U=w.U)
+        torch.cuda.synchronize()
+        ms[name] = ctx.kernel_time_ms()[0]
+    ctx.enable_kernel_timer(False)
+    rel = ((o32 - o64).abs() / o64.abs()).cpu().numpy()
+    return {"workload": w.name, "kernel_ms_f64": ms["f64"], "kernel_ms_f32": ms["f32"], "uplift": ms["f64"] / ms["f32"],
+            "configs_per_s_f32": w.batch / (ms["f32"] * 1e-3), "rel_err_vs_f64_median": float(np.median(rel)),
+            "rel_err_vs_f64_p90": float(np.quantile(rel, 0.9)), "kernel": "eval_team_kernel<float>"}
+
+
+def mc_line(torch, runner, flush, eval_kernel_ms):
+    """On-device Metropolis driver: walker updates per second on the headline workload and the cost
+    of a Monte Carlo step against one plain pass of the hot path ("very little overhead")."""
+    w = runner.w
+    if w.kind != "hubbard":
+        return None
+    ctx = runner.ctx
+    xy, tau = runner.xy.clone(), runner.tau.clone()
+    weight = torch.empty(w.batch, dtype=torch.float64, device="cuda")
+    accepted = torch.empty(w.batch, dtype=torch.int64, device="cuda")
+    steps = 10
+    ctx.mc_run(xy, tau, weight, 2, 1, U=w.U, g_diag=w.g_diag)              # warm-up
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    flush.fill_(1)
+    e0.record()
+    ctx.mc_run(xy, tau, weight, steps, 2, U=w.U, g_diag=w.g_diag, d_accepted=accepted)
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1)
+    # one step = 1/(steps+1) of the call (the call also evaluates the initial configurations once)
+    per_step = ms / (steps + 1)
+    e0.record()
+    for _ in range(steps + 1):
+        runner.step()
+    e1.record()
+    torch.cuda.synchronize()
+    plain = e0.elapsed_time(e1) / (steps + 1)
+    return {"workload": w.name, "walkers": w.batch, "steps": steps, "ms_per_step": per_step,
+            "walker_updates_per_s": w.batch / (per_step * 1e-3), "plain_hot_path_ms": plain,
+            "overhead_vs_plain_pass": per_step / plain - 1.0,
+            "acceptance": float(accepted.double().mean().item() / steps)}
 
 
 def main():
