@@ -37,7 +37,8 @@ if ROOT not in sys.path:
 
 import numpy as np  # noqa: E402
 
-from paper_2501_00675_b200 import sharding, workloads as wl  # noqa: E402
+from paper_2501_00675_b200 import sharding
+from harness import workloads as wl  # noqa: E402
 
 METRIC = "order-n configurations/sec"
 UNIT = "configurations/s"

@@ -1,7 +1,4 @@
-"""B200-native combinatorial-summation (CoS) evaluation of connected Feynman-diagram sums.
+"""B200-native combinatorial-summation (CoS) evaluation: ctypes binding `api` over the C-ABI library libcos_b200.so
+(include/cos.h), its in-tree build script `build`, and the batch-sharding helpers `sharding`.  See DESIGN.md."""
 
-Public API (thin ctypes binding over the C-ABI library `libcos_b200.so`, see include/cos.h):
-    from paper_2501_00675_b200 import api      # cos_create, cos_build_G, cos_eval_connected, ...
-    from paper_2501_00675_b200 import workloads  # seeded synthetic inputs (numpy only)
-"""
-__all__ = ["api", "workloads"]
+__all__ = ["api", "build", "sharding"]

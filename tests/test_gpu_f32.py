@@ -64,7 +64,8 @@ def test_f32_survives_small_greens_functions(oracle_mod):
 def test_f32_accuracy_experiment_order_10(oracle_mod):
     """The paper's experiment ("order of 10^-5 % error ... order 10 configuration") on cfg3-style inputs."""
     import torch
-    from paper_2501_00675_b200 import api, workloads as wl
+    from paper_2501_00675_b200 import api
+    from harness import workloads as wl
     w = wl.baseline_config(3, batch=4096)
     G, _ = oracle_mod.build_G(w.xy, w.tau, w.table, None, w.beta, w.g_diag)
     ref_all, ref_conn = oracle_mod.eval_all_connected(G, None, U=w.U)

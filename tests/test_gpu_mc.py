@@ -14,7 +14,8 @@ TIE = 1e-9          # |margin| below this: a decision another FP64 summation ord
                                              (11, 40, 8), (14, 6, 4)])
 def test_mc_matches_oracle(oracle_mod, n, walkers, steps):
     import torch
-    from paper_2501_00675_b200 import api, build, workloads as wl
+    from paper_2501_00675_b200 import api, build
+    from harness import workloads as wl
     build.build()
     L, beta, ntau, U, seed = 8, 4.0, 65, 2.5, 1234567 + n
     table = wl.g0_table(L, beta, -0.4, ntau)

@@ -54,7 +54,7 @@ def _workload_mats(oracle_mod, w):
 # ------------------------------------------------------------------------------------------ a1
 @pytest.mark.parametrize("cfg,batch", [(1, 64), (2, 4096), (3, 2048), (4, 1024)])
 def test_build_G_bit_exact(torch_mod, ctx, oracle_mod, cfg, batch):
-    from paper_2501_00675_b200 import workloads as wl
+    from harness import workloads as wl
     torch = torch_mod
     w = wl.baseline_config(cfg, batch=batch)
     ref_up, ref_dn = oracle_mod.build_G(w.xy, w.tau, w.table, None, w.beta, 0.0)
@@ -136,7 +136,7 @@ def test_eval_many_teams_per_cta(torch_mod, ctx, oracle_mod, n, nsp):
 @pytest.mark.parametrize("cfg,batch", [(1, 64), (2, 4096), (3, 1024), (4, 256), (5, 16)])
 def test_eval_baseline_configs(torch_mod, ctx, oracle_mod, cfg, batch):
     """BASELINE.json configs (sizes the oracle finishes in seconds), element by element."""
-    from paper_2501_00675_b200 import workloads as wl
+    from harness import workloads as wl
     w = wl.baseline_config(cfg, batch=batch)
     Gup, Gdn, U, u = _workload_mats(oracle_mod, w)
     for which in ("all", "connected"):
@@ -153,7 +153,7 @@ def test_eval_baseline_configs(torch_mod, ctx, oracle_mod, cfg, batch):
 
 
 def test_fused_xt_and_host_paths(torch_mod, ctx, oracle_mod):
-    from paper_2501_00675_b200 import workloads as wl
+    from harness import workloads as wl
     torch = torch_mod
     w = wl.baseline_config(3, batch=300)
     Gup, _ = oracle_mod.build_G(w.xy, w.tau, w.table, None, w.beta, 0.0)
@@ -246,7 +246,8 @@ def test_full_size_sampled_outputs(torch_mod, oracle_mod, cfg, nsample):
     """BASELINE.json configs at their FULL batch, through the entry point and launch configuration bench.py
     times (cos_eval_connected_xt for the Hubbard configs: build_G + evaluation over the whole batch;
     cos_eval_connected for config 5), checked on a seeded sample of outputs the oracle computes one by one."""
-    from paper_2501_00675_b200 import api, workloads as wl
+    from paper_2501_00675_b200 import api
+    from harness import workloads as wl
     torch = torch_mod
     w = wl.baseline_config(cfg)                       # full batch: 4096 / 16384 / 4096 / 512
     out = torch.empty(w.batch, dtype=torch.float64, device="cuda")

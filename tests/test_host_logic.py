@@ -29,7 +29,8 @@ _WORKER = r'''
 import os, sys
 sys.path.insert(0, os.environ["COS_ROOT"])
 import numpy as np, torch, torch.distributed as dist
-from paper_2501_00675_b200 import sharding, workloads as wl
+from paper_2501_00675_b200 import sharding
+from harness import workloads as wl
 import oracle
 dist.init_process_group("gloo")
 rank, _, world = sharding.env_rank_world()
@@ -69,7 +70,7 @@ def test_parity_rule_accepts_fp64_reorderings_and_rejects_errors(oracle_mod):
     a result that is wrong in the 8th digit must fail it."""
     sys.path.insert(0, os.path.join(ROOT, "tests"))
     from parity_util import CLUSTERED_EXCEPTION_FRACTION, check_parity
-    from paper_2501_00675_b200 import workloads as wl
+    from harness import workloads as wl
     w = wl.baseline_config(4, batch=512)                       # clustered times: the hardest config
     G, _ = oracle_mod.build_G(w.xy, w.tau, w.table, None, w.beta, 0.0)
     p = np.random.default_rng(0).permutation(w.n)

@@ -8,7 +8,7 @@ import os
 import numpy as np
 import pytest
 
-from paper_2501_00675_b200 import workloads as wl
+from harness import workloads as wl
 
 GOLD = os.path.join(os.path.dirname(__file__), "golden")
 

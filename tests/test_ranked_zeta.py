@@ -9,7 +9,7 @@ The experiment (oracle/ranked_zeta.py, numpy FP64, no GPU) is compared with the 
 import numpy as np
 
 from oracle import ranked_zeta
-from paper_2501_00675_b200 import workloads as wl
+from harness import workloads as wl
 
 
 def test_ranked_zeta_agrees_on_well_conditioned_inputs(oracle_mod):
