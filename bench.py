@@ -45,6 +45,14 @@ UNIT = "configurations/s"
 HEADLINE_CFG = 3          # BASELINE.json configs[2]: n=10, batch 16384 (largest batch at n >= 10)
 
 
+def config_dict(w):
+    """The `config` object of the JSON line: the same for both arms (the reference arm times a bounded sample of this
+    workload and says so in `cpu_baseline.sample`)."""
+    return {"workload": w.name, "n": w.n, "batch_per_gpu": w.batch, "species_propagations": 1, "g_diag": w.g_diag,
+            "l2": "256 MiB device buffer rewritten between steps, outside the per-step event pairs",
+            "entry": "cos_eval_connected_xt" if w.kind == "hubbard" else "cos_eval_connected"}
+
+
 def parse_args():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -260,7 +268,7 @@ def run_reference(args):
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
-        "data": "synthetic", "config": {"workload": w.name, "n": w.n, "batch": w.batch, "sample_per_step": sample},
+        "data": "synthetic", "config": config_dict(w),
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": int(cores), "kind": "oracle", "sample": desc},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -398,9 +406,7 @@ def run_ours(args):
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": w.name, "n": w.n, "batch_per_gpu": w.batch, "species_propagations": runner.n_species,
-                   "g_diag": w.g_diag, "l2": "256 MiB device buffer rewritten between steps, outside the per-step event pairs",
-                   "entry": "cos_eval_connected_xt" if w.kind == "hubbard" else "cos_eval_connected"},
+        "config": config_dict(w),
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
         "gpu_launches": launches,
         "clocks": clocks,
