@@ -115,8 +115,8 @@ int cos_eval_connected_xt_host(cos_ctx* ctx, int n, long long batch, const int* 
  * the result is homogeneous of degree 2n in G, so it is multiplied by the inverse power on output -- without this
  * the products of ten small Green's functions leave the FP32 range), rounds G and u once to FP32 into buffers of its
  * own, and every later operation -- propagation, combine, connected reduction -- is FP32; the result is widened to
- * FP64 on output.  Built for orders 1..10
- * (COS_EINVAL above).  NOTE (reading R5): this build obtains `connected` by subtracting disconnected
+ * FP64 on output.  All orders 1..16 (every kernel family is instantiated for float).
+ * NOTE (reading R5): this build obtains `connected` by subtracting disconnected
  * parts, so its FP32 error is about eps_32 * |D| / |C| per configuration, larger than the paper's figure, which is
  * for a subtraction-free graph; DESIGN.md reports the measured distribution. */
 int cos_eval_all_f32(cos_ctx* ctx, int n, long long batch, const double* d_Gup, const double* d_Gdn,

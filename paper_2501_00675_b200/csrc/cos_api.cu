@@ -144,10 +144,10 @@ int do_eval(cos_ctx* c, int n, long long batch, const double* gup, const double*
         a.tabs = c->team_tabs[n];
     } else if (n >= kPairGlobalMinN - 1) {   // item descriptors of the global-record pair kernel, built on first use
         if (!c->team_tabs[n]) {
-            const size_t bytes = ((size_t)1 << (n - kPairB)) * kPairDscWords * sizeof(uint32_t);
+            const size_t bytes = ((size_t)1 << (n - f64::kPairB)) * f64::kPairDscWords * sizeof(uint32_t);
             unsigned char* buf = nullptr;
             if (alloc_dev(c, (void**)&buf, bytes) != COS_OK) return COS_ENOMEM;
-            pair_tables_kernel<<<32, 256, 0, c->stream>>>(n, reinterpret_cast<uint32_t*>(buf));
+            f64::pair_tables_kernel<<<32, 256, 0, c->stream>>>(n, reinterpret_cast<uint32_t*>(buf));
             COS_CUDA(c, cudaGetLastError());
             c->team_tabs[n] = buf;
         }
@@ -208,7 +208,6 @@ __global__ void __launch_bounds__(256) unscale_f32_kernel(int n, long long batch
 int do_eval_f32(cos_ctx* c, int n, long long batch, const double* gup, const double* gdn, const double* u, double U,
                 double* out, int connected)
 {
-    if (n > kF32MaxN) return COS_EINVAL;
     if (batch == 0) return COS_OK;
     const bool two = gdn != gup;
     const size_t nn = (size_t)batch * n * n, nu = u ? (size_t)batch * n : 0;
@@ -238,6 +237,24 @@ int do_eval_f32(cos_ctx* c, int n, long long batch, const double* gup, const dou
             c->team_tabs32[n] = buf;
         }
         a.tabs = c->team_tabs32[n];
+    } else if (n >= kPairGlobalMinN - 1) {   // item descriptors of the global-record pair kernel (integers: shared with FP64)
+        if (!c->team_tabs[n]) {
+            const size_t bytes = ((size_t)1 << (n - f64::kPairB)) * f64::kPairDscWords * sizeof(uint32_t);
+            unsigned char* buf = nullptr;
+            if (alloc_dev(c, (void**)&buf, bytes) != COS_OK) return COS_ENOMEM;
+            f64::pair_tables_kernel<<<32, 256, 0, c->stream>>>(n, reinterpret_cast<uint32_t*>(buf));
+            COS_CUDA(c, cudaGetLastError());
+            c->team_tabs[n] = buf;
+        }
+        a.tabs = c->team_tabs[n];
+    }
+    const size_t per_cta = pair_global_rec_doubles(n);      // elements; the FP64-sized block is simply half used
+    if (per_cta) {
+        const int ctas = eval_max_ctas(batch, c->num_sms);
+        rc = grow(c, (void**)&c->scratch, &c->scratch_bytes, per_cta * sizeof(double) * (size_t)ctas);
+        if (rc != COS_OK) return rc;
+        a.scratch = c->scratch;
+        a.scratch_stride = per_cta;
     }
     const bool t = timer_begin(c);
     int launches = 0;

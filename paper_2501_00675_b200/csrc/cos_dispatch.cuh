@@ -4,13 +4,13 @@
 //   n = 11..13 (one species <= 13,
 //               two species <= 12)  eval_pair_kernel      (items split over lane pairs, shared memory)
 //   n = 14..16, two species n = 13  eval_pair_kernel<..., GLOBAL = true>  (records in per-CTA global scratch)
+// The FP32 entry points dispatch the same shapes from namespace f32 (float records).
 // The generic kernel also runs any order when the context is told to (cos_debug_force_generic): it is the
 // in-library cross-check of the tuned kernels, not a fallback for another device.
 #pragma once
 #include "cos_common.cuh"
 #include "cos_kernels_generic.cuh"
 #include "cos_kernels_typed.cuh"
-#include "cos_kernels_pair.cuh"
 
 namespace cosb {
 
@@ -55,18 +55,25 @@ inline TeamChoice32 team_choice_f32(int n, int nsp)
     if (n == 8) return {f32::eval_team_kernel<16, 160, 3>, f32::team_dims<16>(n, nsp)};
     return {f32::eval_team_kernel<32, 192, 2>, f32::team_dims<32>(n, nsp)};
 }
-constexpr int kF32MaxN = kTeamMaxN;       // the FP32 variant is built for orders 1..10 (generic + team kernels)
 
 // ---- pair kernel (orders 11..13): the team mapping with every item split over a lane pair ----
 constexpr int kPairMinN = 11, kPairMaxN = 13;
-using PairKernel = void (*)(EvalArgs, PairDims);
-struct PairChoice { PairKernel fn; PairDims d; };
+using PairKernel = void (*)(EvalArgs, f64::PairDims);
+struct PairChoice { PairKernel fn; f64::PairDims d; };
+using PairKernel32 = void (*)(EvalArgs, f32::PairDims);
+struct PairChoice32 { PairKernel32 fn; f32::PairDims d; };
 inline bool uses_pair(int n, int nsp) { return n >= kPairMinN && n <= (nsp == 1 ? kPairMaxN : kPairMaxN - 1); }
 inline PairChoice pair_choice(int n, int nsp)
 {
-    if (n == 13) return {eval_pair_kernel<1, 512, 1, 10>, pair_dims<1>(n, 1)};   // one species only
-    if (n == 12) return {eval_pair_kernel<2, 512, 1, 9>, pair_dims<2>(n, nsp)};
-    return {eval_pair_kernel<4, 512, 1, 8>, pair_dims<4>(n, nsp, 512)};
+    if (n == 13) return {f64::eval_pair_kernel<1, 512, 1, 10>, f64::pair_dims<1>(n, 1)};   // one species only
+    if (n == 12) return {f64::eval_pair_kernel<2, 512, 1, 9>, f64::pair_dims<2>(n, nsp)};
+    return {f64::eval_pair_kernel<4, 512, 1, 8>, f64::pair_dims<4>(n, nsp, 512)};
+}
+inline PairChoice32 pair_choice_f32(int n, int nsp)       // float records: twice the instances fit
+{
+    if (n == 13) return {f32::eval_pair_kernel<2, 512, 1, 10>, f32::pair_dims<2>(n, nsp, 512)};
+    if (n == 12) return {f32::eval_pair_kernel<4, 512, 1, 9>, f32::pair_dims<4>(n, nsp, 512)};
+    return {f32::eval_pair_kernel<4, 512, 1, 8>, f32::pair_dims<4>(n, nsp, 512)};
 }
 
 // ---- pair kernel on global records (orders 14..16; two species from 13): Z / frontier / reduction arrays in L2 scratch ----
@@ -77,8 +84,13 @@ inline bool uses_pair_global(int n, int nsp)
 }
 inline PairChoice pair_global_choice(int n, int nsp = 1)
 {
-    if (nsp == 2) return {eval_pair_kernel<2, kPairGlobalThreads, 1, 8, true>, pair_dims_global<2>(n, kPairGlobalThreads, 2)};
-    return {eval_pair_kernel<1, kPairGlobalThreads, 1, 8, true>, pair_dims_global<1>(n, kPairGlobalThreads)};
+    if (nsp == 2) return {f64::eval_pair_kernel<2, kPairGlobalThreads, 1, 8, true>, f64::pair_dims_global<2>(n, kPairGlobalThreads, 2)};
+    return {f64::eval_pair_kernel<1, kPairGlobalThreads, 1, 8, true>, f64::pair_dims_global<1>(n, kPairGlobalThreads)};
+}
+inline PairChoice32 pair_global_choice_f32(int n, int nsp = 1)
+{
+    if (nsp == 2) return {f32::eval_pair_kernel<2, kPairGlobalThreads, 1, 8, true>, f32::pair_dims_global<2>(n, kPairGlobalThreads, 2)};
+    return {f32::eval_pair_kernel<1, kPairGlobalThreads, 1, 8, true>, f32::pair_dims_global<1>(n, kPairGlobalThreads)};
 }
 inline size_t pair_global_rec_doubles(int n)
 {
@@ -116,10 +128,16 @@ inline cudaError_t configure_kernels(int smem_optin)
     for (int n = kPairMinN; n <= kPairMaxN; ++n) {
         e = cudaFuncSetAttribute(pair_choice(n, 1).fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
         if (e != cudaSuccess) return e;
+        e = cudaFuncSetAttribute(pair_choice_f32(n, 1).fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
+        if (e != cudaSuccess) return e;
     }
-    e = cudaFuncSetAttribute(pair_global_choice(kPairGlobalMinN, 1).fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
-    if (e != cudaSuccess) return e;
-    return cudaFuncSetAttribute(pair_global_choice(kPairGlobalMinN, 2).fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
+    for (int nsp = 1; nsp <= 2; ++nsp) {
+        e = cudaFuncSetAttribute(pair_global_choice(kPairGlobalMinN, nsp).fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
+        if (e != cudaSuccess) return e;
+        e = cudaFuncSetAttribute(pair_global_choice_f32(kPairGlobalMinN, nsp).fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
+        if (e != cudaSuccess) return e;
+    }
+    return cudaSuccess;
 }
 
 template <class Kernel, class Dims>
@@ -188,7 +206,17 @@ inline cudaError_t dispatch_eval_f32(const EvalArgs& a, cudaStream_t stream, int
         *name = "eval_team_kernel<float>";
         return launch_persistent(tc.fn, tc.d, a, (a.batch * nsp + tc.d.C - 1) / tc.d.C, 0, num_sms, stream);
     }
-    if (a.n > kF32MaxN) return cudaErrorInvalidValue;
+    if (uses_pair(a.n, nsp)) {
+        const PairChoice32 tc = pair_choice_f32(a.n, nsp);
+        *name = "eval_pair_kernel<float>";
+        return launch_persistent(tc.fn, tc.d, a, (a.batch * nsp + tc.d.C - 1) / tc.d.C, 0, num_sms, stream);
+    }
+    if (uses_pair_global(a.n, nsp)) {
+        const PairChoice32 tc = pair_global_choice_f32(a.n, nsp);
+        if (a.scratch == nullptr || (size_t)tc.d.rec_doubles > a.scratch_stride) return cudaErrorInvalidValue;
+        *name = "eval_pair_kernel<float>(global)";
+        return launch_persistent(tc.fn, tc.d, a, a.batch, eval_max_ctas(a.batch, num_sms), num_sms, stream);
+    }
     const size_t smem = generic_smem_bytes(a.n, nsp, sizeof(float));
     int per_sm = 1;
     cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, f32::eval_generic_kernel<kGenericThreads>,

@@ -24,6 +24,7 @@ __device__ __forceinline__ real2 make_real2(real a, real b) { return make_double
 __device__ __forceinline__ const real* in_real(const double* p) { return p; }
 #include "cos_eval_generic.inc"
 #include "cos_eval_team.inc"
+#include "cos_eval_pair.inc"
 }  // namespace f64
 
 namespace f32 {
@@ -33,6 +34,7 @@ __device__ __forceinline__ real2 make_real2(real a, real b) { return make_float2
 __device__ __forceinline__ const real* in_real(const double* p) { return reinterpret_cast<const real*>(p); }
 #include "cos_eval_generic.inc"
 #include "cos_eval_team.inc"
+#include "cos_eval_pair.inc"
 }  // namespace f32
 
 }  // namespace cosb
