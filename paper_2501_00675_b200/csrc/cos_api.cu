@@ -142,7 +142,7 @@ int do_eval(cos_ctx* c, int n, long long batch, const double* gup, const double*
             c->team_tabs[n] = buf;
         }
         a.tabs = c->team_tabs[n];
-    } else if (n >= kPairGlobalMinN - 1) {   // item descriptors of the global-record pair kernel, built on first use
+    } else if (n >= kPairMinN) {   // item descriptors of the global-record pair kernel, built on first use
         if (!c->team_tabs[n]) {
             const size_t bytes = ((size_t)1 << (n - f64::kPairB)) * f64::kPairDscWords * sizeof(uint32_t);
             unsigned char* buf = nullptr;
@@ -154,7 +154,7 @@ int do_eval(cos_ctx* c, int n, long long batch, const double* gup, const double*
         a.tabs = c->team_tabs[n];
     }
     // global scratch for the orders whose frontier does not fit in shared memory
-    const size_t per_cta = eval_scratch_doubles(n, c->smem_optin, c->force_generic);
+    const size_t per_cta = eval_scratch_doubles(n, gdn == gup ? 1 : 2, batch, c->num_sms, c->smem_optin, c->force_generic, false);
     if (per_cta) {
         const int ctas = eval_max_ctas(batch, c->num_sms);
         int rc = grow(c, (void**)&c->scratch, &c->scratch_bytes, per_cta * sizeof(double) * (size_t)ctas);
@@ -237,7 +237,7 @@ int do_eval_f32(cos_ctx* c, int n, long long batch, const double* gup, const dou
             c->team_tabs32[n] = buf;
         }
         a.tabs = c->team_tabs32[n];
-    } else if (n >= kPairGlobalMinN - 1) {   // item descriptors of the global-record pair kernel (integers: shared with FP64)
+    } else if (n >= kPairMinN) {   // item descriptors of the global-record pair kernel (integers: shared with FP64)
         if (!c->team_tabs[n]) {
             const size_t bytes = ((size_t)1 << (n - f64::kPairB)) * f64::kPairDscWords * sizeof(uint32_t);
             unsigned char* buf = nullptr;
@@ -248,7 +248,7 @@ int do_eval_f32(cos_ctx* c, int n, long long batch, const double* gup, const dou
         }
         a.tabs = c->team_tabs[n];
     }
-    const size_t per_cta = pair_global_rec_doubles(n);      // elements; the FP64-sized block is simply half used
+    const size_t per_cta = eval_scratch_doubles(n, two ? 2 : 1, batch, c->num_sms, c->smem_optin, false, true);   // elements
     if (per_cta) {
         const int ctas = eval_max_ctas(batch, c->num_sms);
         rc = grow(c, (void**)&c->scratch, &c->scratch_bytes, per_cta * sizeof(double) * (size_t)ctas);
@@ -259,7 +259,7 @@ int do_eval_f32(cos_ctx* c, int n, long long batch, const double* gup, const dou
     const bool t = timer_begin(c);
     int launches = 0;
     const char* name = nullptr;
-    cudaError_t e = dispatch_eval_f32(a, c->stream, c->num_sms, &launches, &name);
+    cudaError_t e = dispatch_eval_f32(a, c->stream, c->num_sms, c->smem_optin, &launches, &name);
     if (t) timer_end(c);
     if (e != cudaSuccess) return fail_cuda(c, e);
     unscale_f32_kernel<<<blocks, 256, 0, c->stream>>>(n, batch, kexp, out);

@@ -1,10 +1,10 @@
 // cos_dispatch.cuh -- picks the kernel variant for an evaluation launch and sizes its resources.
 //   n = 1..4                        eval_generic_kernel   (one thread per node, frontier in shared memory)
 //   n = 5..10                       eval_team_kernel      (C instances per CTA, thread-bit register tiles)
-//   n = 11..13 (one species <= 13,
-//               two species <= 12)  eval_pair_kernel      (items split over lane pairs, shared memory)
-//   n = 14..16, two species n = 13  eval_pair_kernel<..., GLOBAL = true>  (records in per-CTA global scratch)
-// The FP32 entry points dispatch the same shapes from namespace f32 (float records).
+//   n = 11 (one species, FP64)      eval_pair_kernel      (items split over lane pairs, records in shared memory)
+//   n = 11..16 otherwise            eval_pair_kernel<..., GLOBAL = true>  (records in per-CTA global scratch, teams of
+//                                   1..8 instances per CTA chosen by pair_plan)
+// The FP32 entry points dispatch the same kernels from namespace f32 (float records).
 // The generic kernel also runs any order when the context is told to (cos_debug_force_generic): it is the
 // in-library cross-check of the tuned kernels, not a fallback for another device.
 #pragma once
@@ -56,54 +56,89 @@ inline TeamChoice32 team_choice_f32(int n, int nsp)
     return {f32::eval_team_kernel<32, 192, 2>, f32::team_dims<32>(n, nsp)};
 }
 
-// ---- pair kernel (orders 11..13): the team mapping with every item split over a lane pair ----
-constexpr int kPairMinN = 11, kPairMaxN = 13;
-using PairKernel = void (*)(EvalArgs, f64::PairDims);
-struct PairChoice { PairKernel fn; f64::PairDims d; };
-using PairKernel32 = void (*)(EvalArgs, f32::PairDims);
-struct PairChoice32 { PairKernel32 fn; f32::PairDims d; };
-inline bool uses_pair(int n, int nsp) { return n >= kPairMinN && n <= (nsp == 1 ? kPairMaxN : kPairMaxN - 1); }
-inline PairChoice pair_choice(int n, int nsp)
+// ---- pair kernel (orders 11..16): the team mapping with every item split over a lane pair ----
+// Two homes for the records (Z, frontier, reduction arrays): shared memory, or a per-CTA block of global scratch that
+// stays in L1/L2.  The global variant is not limited by the 227 KB of an SM, so a CTA can work on a team of several
+// configurations and every level exposes that many times more items per barrier; measured (round 2, product build,
+// kernel ms, shared C / global C = 1 / best global C):
+//   one species   n=12: 0.549 / - / 0.490 (C=8)   n=13: 0.388 / 0.42 / 0.333 (C=4)   n=14: - / 0.864 / 0.846 (C=2)
+//                 n=15: - / 1.214 / 1.107 (C=2)   n=16: - / 1.740 / 1.577 (C=2)      n=11: 0.221 / - / 0.226 (C=8)
+//   two species   n=11: 0.376 / - / 0.348 (C=8)   n=12: 0.973 / - / 0.684 (C=8)      n=13: - / 0.571 (C=2) / 0.480 (C=4)
+//                 n=15: - / 1.705 (C=2) / 1.500 (C=4)   n=16: - / 2.280 (C=2) / 1.992 (C=4)
+constexpr int kPairMinN = 11, kPairGlobalThreads = 512;
+struct PairPlan {
+    bool global;     // records in global scratch
+    int C;           // instances per team
+};
+// The plan of one launch: where the records live and how many instances a CTA takes at a time.
+inline PairPlan pair_plan(int n, int nsp, long long batch, int num_sms, bool f32)
 {
-    if (n == 13) return {f64::eval_pair_kernel<1, 512, 1, 10>, f64::pair_dims<1>(n, 1)};   // one species only
-    if (n == 12) return {f64::eval_pair_kernel<2, 512, 1, 9>, f64::pair_dims<2>(n, nsp)};
-    return {f64::eval_pair_kernel<4, 512, 1, 8>, f64::pair_dims<4>(n, nsp, 512)};
-}
-inline PairChoice32 pair_choice_f32(int n, int nsp)       // float records: twice the instances fit
-{
-    if (n == 13) return {f32::eval_pair_kernel<2, 512, 1, 10>, f32::pair_dims<2>(n, nsp, 512)};
-    if (n == 12) return {f32::eval_pair_kernel<4, 512, 1, 9>, f32::pair_dims<4>(n, nsp, 512)};
-    return {f32::eval_pair_kernel<4, 512, 1, 8>, f32::pair_dims<4>(n, nsp, 512)};
-}
-
-// ---- pair kernel on global records (orders 14..16; two species from 13): Z / frontier / reduction arrays in L2 scratch ----
-constexpr int kPairGlobalMinN = 14, kPairGlobalThreads = 512;
-inline bool uses_pair_global(int n, int nsp)
-{
-    return n <= kMaxN && (nsp == 1 ? n >= kPairGlobalMinN : n >= kPairGlobalMinN - 1);
-}
-inline PairChoice pair_global_choice(int n, int nsp = 1)
-{
-    if (nsp == 2) return {f64::eval_pair_kernel<2, kPairGlobalThreads, 1, 8, true>, f64::pair_dims_global<2>(n, kPairGlobalThreads, 2)};
-    return {f64::eval_pair_kernel<1, kPairGlobalThreads, 1, 8, true>, f64::pair_dims_global<1>(n, kPairGlobalThreads)};
-}
-inline PairChoice32 pair_global_choice_f32(int n, int nsp = 1)
-{
-    if (nsp == 2) return {f32::eval_pair_kernel<2, kPairGlobalThreads, 1, 8, true>, f32::pair_dims_global<2>(n, kPairGlobalThreads, 2)};
-    return {f32::eval_pair_kernel<1, kPairGlobalThreads, 1, 8, true>, f32::pair_dims_global<1>(n, kPairGlobalThreads)};
-}
-inline size_t pair_global_rec_doubles(int n)
-{
-    if (n < kPairGlobalMinN - 1 || n > kMaxN) return 0;
-    const size_t a = (size_t)pair_global_choice(n, 1).d.rec_doubles, b = (size_t)pair_global_choice(n, 2).d.rec_doubles;
-    return a > b ? a : b;
+    PairPlan p{true, 2};
+    if (!f32) {
+        if (n == 11) p = (nsp == 1) ? PairPlan{false, 4} : PairPlan{true, 8};
+        else if (n == 12) p = {true, 8};
+        else if (n == 13) p = {true, 4};
+        else if (n == 14) p = {true, 2};
+        else p = {true, nsp == 1 ? 2 : 4};
+    } else {                           // float records: measured best on global records at every order
+        p = {true, n <= 12 ? 8 : 4};   //   (n=11: 0.154 ms against 0.186 in shared memory, n=12: 0.296 / 0.327, n=13: 0.210 / 0.245)
+    }
+    // a team of C instances per CTA: shrink it only when more than half of the SMs would get no team at all
+    // (n = 16, batch 256: 128 teams of 2 on 148 SMs measured 1.58 ms against 1.74 ms for 256 teams of 1)
+    if (p.global)
+        while (p.C > nsp && (batch * nsp + p.C - 1) / p.C < num_sms / 2) p.C /= 2;
+    return p;
 }
 
-// Doubles of global scratch per CTA (0: everything lives in shared memory).
-inline size_t eval_scratch_doubles(int n, int smem_optin, bool force_generic)
+// Precision traits: the same launch table serves cosb::f64 and cosb::f32.
+struct Prec64 {
+    static constexpr bool kF32 = false;
+    using Dims = f64::PairDims;
+    template <int C, int NC, bool G> static auto kernel() { return f64::eval_pair_kernel<C, 512, 1, NC, G>; }
+    template <int C> static Dims dims(int n, int nsp) { return f64::pair_dims<C>(n, nsp, 512); }
+    template <int C> static Dims dims_global(int n, int nsp) { return f64::pair_dims_global<C>(n, kPairGlobalThreads, nsp); }
+};
+struct Prec32 {
+    static constexpr bool kF32 = true;
+    using Dims = f32::PairDims;
+    template <int C, int NC, bool G> static auto kernel() { return f32::eval_pair_kernel<C, 512, 1, NC, G>; }
+    template <int C> static Dims dims(int n, int nsp) { return f32::pair_dims<C>(n, nsp, 512); }
+    template <int C> static Dims dims_global(int n, int nsp) { return f32::pair_dims_global<C>(n, kPairGlobalThreads, nsp); }
+};
+
+// Calls f(kernel, dims) for the kernel instance of plan p at order n (false: no such instance).
+template <class P, class F>
+inline bool with_pair_instance(const PairPlan& p, int n, int nsp, F&& f)
+{
+    if (p.global) {
+        switch (p.C) {
+            case 1: f(P::template kernel<1, 8, true>(), P::template dims_global<1>(n, nsp)); return true;
+            case 2: f(P::template kernel<2, 8, true>(), P::template dims_global<2>(n, nsp)); return true;
+            case 4: f(P::template kernel<4, 8, true>(), P::template dims_global<4>(n, nsp)); return true;
+            case 8: f(P::template kernel<8, 8, true>(), P::template dims_global<8>(n, nsp)); return true;
+            default: return false;
+        }
+    }
+    if (n == 11 && p.C == 4) { f(P::template kernel<4, 8, false>(), P::template dims<4>(n, nsp)); return true; }
+    return false;
+}
+
+// Elements of global scratch per CTA for plan p (0: shared memory).
+template <class P>
+inline size_t pair_plan_scratch(const PairPlan& p, int n, int nsp)
+{
+    size_t v = 0;
+    if (p.global) with_pair_instance<P>(p, n, nsp, [&](auto, const typename P::Dims& d) { v = (size_t)d.rec_doubles; });
+    return v;
+}
+
+// Elements of global scratch per CTA (0: everything lives in shared memory).
+inline size_t eval_scratch_doubles(int n, int nsp, long long batch, int num_sms, int smem_optin, bool force_generic, bool f32)
 {
     if (force_generic) return generic_scratch_doubles(n, smem_optin);
-    return pair_global_rec_doubles(n);
+    if (n < kPairMinN) return 0;
+    const PairPlan p = pair_plan(n, nsp, batch, num_sms, f32);
+    return f32 ? pair_plan_scratch<Prec32>(p, n, nsp) : pair_plan_scratch<Prec64>(p, n, nsp);
 }
 
 inline int eval_max_ctas(long long batch, int num_sms)
@@ -125,18 +160,7 @@ inline cudaError_t configure_kernels(int smem_optin)
         e = cudaFuncSetAttribute(team_choice_f32(n, 1).fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
         if (e != cudaSuccess) return e;
     }
-    for (int n = kPairMinN; n <= kPairMaxN; ++n) {
-        e = cudaFuncSetAttribute(pair_choice(n, 1).fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
-        if (e != cudaSuccess) return e;
-        e = cudaFuncSetAttribute(pair_choice_f32(n, 1).fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
-        if (e != cudaSuccess) return e;
-    }
-    for (int nsp = 1; nsp <= 2; ++nsp) {
-        e = cudaFuncSetAttribute(pair_global_choice(kPairGlobalMinN, nsp).fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
-        if (e != cudaSuccess) return e;
-        e = cudaFuncSetAttribute(pair_global_choice_f32(kPairGlobalMinN, nsp).fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
-        if (e != cudaSuccess) return e;
-    }
+    // every pair-kernel instance the plans can name: the attribute is set on first use (launch_pair), see below
     return cudaSuccess;
 }
 
@@ -155,6 +179,26 @@ inline cudaError_t launch_persistent(Kernel fn, const Dims& d, const EvalArgs& a
     return cudaGetLastError();
 }
 
+// Launches the pair-kernel instance the plan names.  The opt-in shared-memory attribute of an instance is set the
+// first time it is used (a handful of instances per precision; setting it again is harmless).
+template <class P>
+inline cudaError_t launch_pair(const EvalArgs& a, int nsp, int num_sms, int smem_optin, cudaStream_t stream,
+                               const char** name, const char* shared_name, const char* global_name)
+{
+    const PairPlan plan = pair_plan(a.n, nsp, a.batch, num_sms, P::kF32);
+    cudaError_t err = cudaErrorInvalidValue;
+    const bool found = with_pair_instance<P>(plan, a.n, nsp, [&](auto fn, const typename P::Dims& d) {
+        if (plan.global && (a.scratch == nullptr || (size_t)d.rec_doubles > a.scratch_stride)) return;
+        if (d.smem_bytes > (size_t)smem_optin) return;
+        err = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
+        if (err != cudaSuccess) return;
+        const long long teams = (a.batch * nsp + d.C - 1) / d.C;
+        err = launch_persistent(fn, d, a, teams, plan.global ? eval_max_ctas(a.batch, num_sms) : 0, num_sms, stream);
+    });
+    *name = plan.global ? global_name : shared_name;
+    return found ? err : cudaErrorInvalidValue;
+}
+
 inline cudaError_t dispatch_eval(const EvalArgs& a, cudaStream_t stream, int num_sms, int smem_optin,
                                  bool force_generic, int* launches, const char** name)
 {
@@ -165,16 +209,8 @@ inline cudaError_t dispatch_eval(const EvalArgs& a, cudaStream_t stream, int num
         *name = "eval_team_kernel";
         return launch_persistent(tc.fn, tc.d, a, (a.batch * nsp + tc.d.C - 1) / tc.d.C, 0, num_sms, stream);
     }
-    if (!force_generic && uses_pair(a.n, nsp)) {
-        const PairChoice tc = pair_choice(a.n, nsp);
-        *name = "eval_pair_kernel";
-        return launch_persistent(tc.fn, tc.d, a, (a.batch * nsp + tc.d.C - 1) / tc.d.C, 0, num_sms, stream);
-    }
-    if (!force_generic && uses_pair_global(a.n, nsp)) {
-        const PairChoice tc = pair_global_choice(a.n, nsp);
-        if (a.scratch == nullptr || (size_t)tc.d.rec_doubles > a.scratch_stride) return cudaErrorInvalidValue;
-        *name = "eval_pair_kernel(global)";
-        return launch_persistent(tc.fn, tc.d, a, a.batch, eval_max_ctas(a.batch, num_sms), num_sms, stream);
+    if (!force_generic && a.n >= kPairMinN) {
+        return launch_pair<Prec64>(a, nsp, num_sms, smem_optin, stream, name, "eval_pair_kernel", "eval_pair_kernel(global)");
     }
     const bool use_global = generic_needs_global(a.n, smem_optin);
     if (use_global && a.scratch == nullptr) return cudaErrorInvalidValue;
@@ -197,7 +233,8 @@ inline cudaError_t dispatch_eval(const EvalArgs& a, cudaStream_t stream, int num
 
 // FP32 variant: orders 1..4 on the plain kernel, 5..10 on the team kernel, both instantiated for float.  The input
 // pointers of `a` address FP32 copies of G and u (made by the entry point).
-inline cudaError_t dispatch_eval_f32(const EvalArgs& a, cudaStream_t stream, int num_sms, int* launches, const char** name)
+inline cudaError_t dispatch_eval_f32(const EvalArgs& a, cudaStream_t stream, int num_sms, int smem_optin, int* launches,
+                                     const char** name)
 {
     const int nsp = (a.Gdn == a.Gup) ? 1 : 2;
     *launches = 1;
@@ -206,17 +243,8 @@ inline cudaError_t dispatch_eval_f32(const EvalArgs& a, cudaStream_t stream, int
         *name = "eval_team_kernel<float>";
         return launch_persistent(tc.fn, tc.d, a, (a.batch * nsp + tc.d.C - 1) / tc.d.C, 0, num_sms, stream);
     }
-    if (uses_pair(a.n, nsp)) {
-        const PairChoice32 tc = pair_choice_f32(a.n, nsp);
-        *name = "eval_pair_kernel<float>";
-        return launch_persistent(tc.fn, tc.d, a, (a.batch * nsp + tc.d.C - 1) / tc.d.C, 0, num_sms, stream);
-    }
-    if (uses_pair_global(a.n, nsp)) {
-        const PairChoice32 tc = pair_global_choice_f32(a.n, nsp);
-        if (a.scratch == nullptr || (size_t)tc.d.rec_doubles > a.scratch_stride) return cudaErrorInvalidValue;
-        *name = "eval_pair_kernel<float>(global)";
-        return launch_persistent(tc.fn, tc.d, a, a.batch, eval_max_ctas(a.batch, num_sms), num_sms, stream);
-    }
+    if (a.n >= kPairMinN)
+        return launch_pair<Prec32>(a, nsp, num_sms, smem_optin, stream, name, "eval_pair_kernel<float>", "eval_pair_kernel<float>(global)");
     const size_t smem = generic_smem_bytes(a.n, nsp, sizeof(float));
     int per_sm = 1;
     cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, f32::eval_generic_kernel<kGenericThreads>,

@@ -106,7 +106,7 @@ def test_eval_every_order_dense(torch_mod, ctx, oracle_mod, n):
 # generic kernel): this drives the prefetch of the next team's matrices, the re-use of the shared-memory / scratch
 # areas between teams and the ragged last team, for EVERY order, one and two species.
 _MANY = {1: 4741, 2: 4741, 3: 4741, 4: 4741, 5: 28417, 6: 28417, 7: 28417, 8: 14209, 9: 7105, 10: 3553,
-         11: 1777, 12: 889, 13: 450, 14: 450, 15: 450, 16: 450}
+         11: 1777, 12: 2400, 13: 1200, 14: 450, 15: 450, 16: 450}
 
 
 @pytest.mark.parametrize("nsp", [1, 2])
@@ -369,4 +369,7 @@ def test_result_independent_of_batch_position_and_repeatable(torch_mod, ctx, n, 
     # a ragged sub-batch (different team boundaries, fewer CTAs) reproduces the same bits for the configurations it holds
     k = max(1, B // 3 + 1)
     c = _gpu_eval(torch, ctx, Gup[:k], None if Gdn is None else Gdn[:k], 1.0, u[:k], "connected")
-    np.testing.assert_array_equal(c, a[:k])
+    if n <= 10:
+        np.testing.assert_array_equal(c, a[:k])
+    else:       # from order 11 the team size follows the batch (cos_dispatch.cuh: pair_plan), and with it the order in
+        np.testing.assert_allclose(c, a[:k], rtol=1e-10)      # which the reduction sums its partial blocks
