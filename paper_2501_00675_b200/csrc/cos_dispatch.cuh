@@ -69,6 +69,7 @@ constexpr int kPairMinN = 11, kPairGlobalThreads = 512;
 struct PairPlan {
     bool global;     // records in global scratch
     int C;           // instances per team
+    bool red_smem;   // global variant: reduction arrays in shared memory
 };
 // The plan of one launch: where the records live and how many instances a CTA takes at a time.
 inline PairPlan pair_plan(int n, int nsp, long long batch, int num_sms, bool f32)
@@ -78,7 +79,8 @@ inline PairPlan pair_plan(int n, int nsp, long long batch, int num_sms, bool f32
         if (n == 11) p = (nsp == 1) ? PairPlan{false, 4} : PairPlan{true, 8};
         else if (n == 12) p = {true, 8};
         else if (n == 13) p = {true, 4};
-        else if (n == 14) p = {true, 2};
+        else if (n == 14) p = (nsp == 1) ? PairPlan{true, 1, true} : PairPlan{true, 2};   // one instance: its reduction
+                                                                      // arrays (128 KB) fit in shared memory: 0.813 / 0.844 ms
         else p = {true, nsp == 1 ? 2 : 4};
     } else {                           // float records: measured best on global records at every order
         p = {true, n <= 12 ? 8 : 4};   //   (n=11: 0.154 ms against 0.186 in shared memory, n=12: 0.296 / 0.327, n=13: 0.210 / 0.245)
@@ -96,14 +98,14 @@ struct Prec64 {
     using Dims = f64::PairDims;
     template <int C, int NC, bool G> static auto kernel() { return f64::eval_pair_kernel<C, 512, 1, NC, G>; }
     template <int C> static Dims dims(int n, int nsp) { return f64::pair_dims<C>(n, nsp, 512); }
-    template <int C> static Dims dims_global(int n, int nsp) { return f64::pair_dims_global<C>(n, kPairGlobalThreads, nsp); }
+    template <int C> static Dims dims_global(int n, int nsp, bool rs) { return f64::pair_dims_global<C>(n, kPairGlobalThreads, nsp, rs); }
 };
 struct Prec32 {
     static constexpr bool kF32 = true;
     using Dims = f32::PairDims;
     template <int C, int NC, bool G> static auto kernel() { return f32::eval_pair_kernel<C, 512, 1, NC, G>; }
     template <int C> static Dims dims(int n, int nsp) { return f32::pair_dims<C>(n, nsp, 512); }
-    template <int C> static Dims dims_global(int n, int nsp) { return f32::pair_dims_global<C>(n, kPairGlobalThreads, nsp); }
+    template <int C> static Dims dims_global(int n, int nsp, bool rs) { return f32::pair_dims_global<C>(n, kPairGlobalThreads, nsp, rs); }
 };
 
 // Calls f(kernel, dims) for the kernel instance of plan p at order n (false: no such instance).
@@ -112,10 +114,10 @@ inline bool with_pair_instance(const PairPlan& p, int n, int nsp, F&& f)
 {
     if (p.global) {
         switch (p.C) {
-            case 1: f(P::template kernel<1, 8, true>(), P::template dims_global<1>(n, nsp)); return true;
-            case 2: f(P::template kernel<2, 8, true>(), P::template dims_global<2>(n, nsp)); return true;
-            case 4: f(P::template kernel<4, 8, true>(), P::template dims_global<4>(n, nsp)); return true;
-            case 8: f(P::template kernel<8, 8, true>(), P::template dims_global<8>(n, nsp)); return true;
+            case 1: f(P::template kernel<1, 8, true>(), P::template dims_global<1>(n, nsp, p.red_smem)); return true;
+            case 2: f(P::template kernel<2, 8, true>(), P::template dims_global<2>(n, nsp, p.red_smem)); return true;
+            case 4: f(P::template kernel<4, 8, true>(), P::template dims_global<4>(n, nsp, p.red_smem)); return true;
+            case 8: f(P::template kernel<8, 8, true>(), P::template dims_global<8>(n, nsp, p.red_smem)); return true;
             default: return false;
         }
     }
