@@ -76,14 +76,14 @@ inline PairPlan pair_plan(int n, int nsp, long long batch, int num_sms, bool f32
 {
     PairPlan p{true, 2};
     if (!f32) {
-        if (n == 11) p = (nsp == 1) ? PairPlan{false, 4} : PairPlan{true, 8};
+        if (n == 11) p = {true, 16};
         else if (n == 12) p = {true, 8};
         else if (n == 13) p = {true, 4};
         else if (n == 14) p = (nsp == 1) ? PairPlan{true, 1, true} : PairPlan{true, 2};   // one instance: its reduction
                                                                       // arrays (128 KB) fit in shared memory: 0.813 / 0.844 ms
         else p = {true, nsp == 1 ? 2 : 4};
-    } else {                           // float records: measured best on global records at every order
-        p = {true, n <= 12 ? 8 : 4};   //   (n=11: 0.154 ms against 0.186 in shared memory, n=12: 0.296 / 0.327, n=13: 0.210 / 0.245)
+    } else {                           // float records: half the L1/L2 traffic, larger teams pay off
+        p = {true, n <= 12 ? 16 : (n == 13 ? 8 : 4)};
     }
     // a team of C instances per CTA: shrink it only when more than half of the SMs would get no team at all
     // (n = 16, batch 256: 128 teams of 2 on 148 SMs measured 1.58 ms against 1.74 ms for 256 teams of 1)
@@ -118,10 +118,10 @@ inline bool with_pair_instance(const PairPlan& p, int n, int nsp, F&& f)
             case 2: f(P::template kernel<2, 8, true>(), P::template dims_global<2>(n, nsp, p.red_smem)); return true;
             case 4: f(P::template kernel<4, 8, true>(), P::template dims_global<4>(n, nsp, p.red_smem)); return true;
             case 8: f(P::template kernel<8, 8, true>(), P::template dims_global<8>(n, nsp, p.red_smem)); return true;
+            case 16: f(P::template kernel<16, 8, true>(), P::template dims_global<16>(n, nsp, p.red_smem)); return true;
             default: return false;
         }
     }
-    if (n == 11 && p.C == 4) { f(P::template kernel<4, 8, false>(), P::template dims<4>(n, nsp)); return true; }
     return false;
 }
 
