@@ -1,9 +1,8 @@
 // cos_dispatch.cuh -- picks the kernel variant for an evaluation launch and sizes its resources.
 //   n = 1..4                        eval_generic_kernel   (one thread per node, frontier in shared memory)
 //   n = 5..10                       eval_team_kernel      (C instances per CTA, thread-bit register tiles)
-//   n = 11 (one species, FP64)      eval_pair_kernel      (items split over lane pairs, records in shared memory)
-//   n = 11..16 otherwise            eval_pair_kernel<..., GLOBAL = true>  (records in per-CTA global scratch, teams of
-//                                   1..8 instances per CTA chosen by pair_plan)
+//   n = 11..16                      eval_pair_kernel      (items split over lane pairs, records in per-CTA global
+//                                   scratch, teams of 1..16 instances per CTA chosen by pair_plan)
 // The FP32 entry points dispatch the same kernels from namespace f32 (float records).
 // The generic kernel also runs any order when the context is told to (cos_debug_force_generic): it is the
 // in-library cross-check of the tuned kernels, not a fallback for another device.
@@ -57,38 +56,38 @@ inline TeamChoice32 team_choice_f32(int n, int nsp)
 }
 
 // ---- pair kernel (orders 11..16): the team mapping with every item split over a lane pair ----
-// Two homes for the records (Z, frontier, reduction arrays): shared memory, or a per-CTA block of global scratch that
-// stays in L1/L2.  The global variant is not limited by the 227 KB of an SM, so a CTA can work on a team of several
-// configurations and every level exposes that many times more items per barrier; measured (round 2, product build,
-// kernel ms, shared C / global C = 1 / best global C):
-//   one species   n=12: 0.549 / - / 0.490 (C=8)   n=13: 0.388 / 0.42 / 0.333 (C=4)   n=14: - / 0.864 / 0.846 (C=2)
-//                 n=15: - / 1.214 / 1.107 (C=2)   n=16: - / 1.740 / 1.577 (C=2)      n=11: 0.221 / - / 0.226 (C=8)
-//   two species   n=11: 0.376 / - / 0.348 (C=8)   n=12: 0.973 / - / 0.684 (C=8)      n=13: - / 0.571 (C=2) / 0.480 (C=4)
-//                 n=15: - / 1.705 (C=2) / 1.500 (C=4)   n=16: - / 2.280 (C=2) / 1.992 (C=4)
-constexpr int kPairMinN = 11, kPairGlobalThreads = 512;
+// The records (Z, frontier, reduction arrays) live in a per-CTA block of global scratch served by L1/L2, so a CTA is
+// not limited by the 227 KB of an SM and works on a TEAM of several instances: every level then exposes that many
+// times more items per block barrier.  Measured (round 2, product build, kernel ms; "shared" = the round-1 kernel
+// with the records in shared memory, since removed):
+//   one species  n=11: shared 0.221, C=8 0.226, C=16 0.216   n=12: shared 0.549, C=4 0.501, C=8 0.490, C=16 0.538
+//                n=13: shared 0.388, C=1 0.42, C=2 0.361, C=4 0.333, C=8 0.355   n=14: C=1 0.864, C=2 0.846, C=4 0.855
+//                n=15: C=1 1.214, C=2 1.107, C=4 1.126        n=16 (batch 256): C=1 1.740, C=2 1.577
+//   two species  n=11: shared 0.376, C=8 0.348, C=16 0.327   n=12: shared 0.973, C=4 0.809, C=8 0.684
+//                n=13: C=2 0.571, C=4 0.480, C=8 0.511        n=15: C=2 1.705, C=4 1.500    n=16: C=2 2.280, C=4 1.992
+//   FP32         n=11: C=8 0.153, C=16 0.128   n=12: C=8 0.294, C=16 0.285   n=13: C=4 0.210, C=8 0.179   n=14: C=4 0.517
+constexpr int kPairMinN = 11, kPairThreads = 512;
 struct PairPlan {
-    bool global;     // records in global scratch
     int C;           // instances per team
-    bool red_smem;   // global variant: reduction arrays in shared memory
+    bool red_smem;   // reduction arrays in shared memory instead of the scratch block
 };
-// The plan of one launch: where the records live and how many instances a CTA takes at a time.
+// The plan of one launch: how many instances a CTA takes at a time.
 inline PairPlan pair_plan(int n, int nsp, long long batch, int num_sms, bool f32)
 {
-    PairPlan p{true, 2};
+    PairPlan p{2, false};
     if (!f32) {
-        if (n == 11) p = {true, 16};
-        else if (n == 12) p = {true, 8};
-        else if (n == 13) p = {true, 4};
-        else if (n == 14) p = (nsp == 1) ? PairPlan{true, 1, true} : PairPlan{true, 2};   // one instance: its reduction
-                                                                      // arrays (128 KB) fit in shared memory: 0.813 / 0.844 ms
-        else p = {true, nsp == 1 ? 2 : 4};
+        if (n == 11) p.C = 16;
+        else if (n == 12) p.C = 8;
+        else if (n == 13) p.C = 4;
+        else if (n == 14) p = (nsp == 1) ? PairPlan{1, true} : PairPlan{2, false};   // one instance: its reduction arrays
+                                                                    // (128 KB) fit in shared memory: 0.813 against 0.844 ms
+        else p.C = (nsp == 1) ? 2 : 4;
     } else {                           // float records: half the L1/L2 traffic, larger teams pay off
-        p = {true, n <= 12 ? 16 : (n == 13 ? 8 : 4)};
+        p.C = n <= 12 ? 16 : (n == 13 ? 8 : 4);
     }
-    // a team of C instances per CTA: shrink it only when more than half of the SMs would get no team at all
+    // shrink the team only when more than half of the SMs would get no team at all
     // (n = 16, batch 256: 128 teams of 2 on 148 SMs measured 1.58 ms against 1.74 ms for 256 teams of 1)
-    if (p.global)
-        while (p.C > nsp && (batch * nsp + p.C - 1) / p.C < num_sms / 2) p.C /= 2;
+    while (p.C > nsp && (batch * nsp + p.C - 1) / p.C < num_sms / 2) { p.C /= 2; p.red_smem = false; }
     return p;
 }
 
@@ -96,41 +95,36 @@ inline PairPlan pair_plan(int n, int nsp, long long batch, int num_sms, bool f32
 struct Prec64 {
     static constexpr bool kF32 = false;
     using Dims = f64::PairDims;
-    template <int C, int NC, bool G> static auto kernel() { return f64::eval_pair_kernel<C, 512, 1, NC, G>; }
-    template <int C> static Dims dims(int n, int nsp) { return f64::pair_dims<C>(n, nsp, 512); }
-    template <int C> static Dims dims_global(int n, int nsp, bool rs) { return f64::pair_dims_global<C>(n, kPairGlobalThreads, nsp, rs); }
+    template <int C> static auto kernel() { return f64::eval_pair_kernel<C, kPairThreads, 1, 8>; }
+    template <int C> static Dims dims(int n, int nsp, bool rs) { return f64::pair_dims<C>(n, kPairThreads, nsp, rs); }
 };
 struct Prec32 {
     static constexpr bool kF32 = true;
     using Dims = f32::PairDims;
-    template <int C, int NC, bool G> static auto kernel() { return f32::eval_pair_kernel<C, 512, 1, NC, G>; }
-    template <int C> static Dims dims(int n, int nsp) { return f32::pair_dims<C>(n, nsp, 512); }
-    template <int C> static Dims dims_global(int n, int nsp, bool rs) { return f32::pair_dims_global<C>(n, kPairGlobalThreads, nsp, rs); }
+    template <int C> static auto kernel() { return f32::eval_pair_kernel<C, kPairThreads, 1, 8>; }
+    template <int C> static Dims dims(int n, int nsp, bool rs) { return f32::pair_dims<C>(n, kPairThreads, nsp, rs); }
 };
 
 // Calls f(kernel, dims) for the kernel instance of plan p at order n (false: no such instance).
 template <class P, class F>
 inline bool with_pair_instance(const PairPlan& p, int n, int nsp, F&& f)
 {
-    if (p.global) {
-        switch (p.C) {
-            case 1: f(P::template kernel<1, 8, true>(), P::template dims_global<1>(n, nsp, p.red_smem)); return true;
-            case 2: f(P::template kernel<2, 8, true>(), P::template dims_global<2>(n, nsp, p.red_smem)); return true;
-            case 4: f(P::template kernel<4, 8, true>(), P::template dims_global<4>(n, nsp, p.red_smem)); return true;
-            case 8: f(P::template kernel<8, 8, true>(), P::template dims_global<8>(n, nsp, p.red_smem)); return true;
-            case 16: f(P::template kernel<16, 8, true>(), P::template dims_global<16>(n, nsp, p.red_smem)); return true;
-            default: return false;
-        }
+    switch (p.C) {
+        case 1: f(P::template kernel<1>(), P::template dims<1>(n, nsp, p.red_smem)); return true;
+        case 2: f(P::template kernel<2>(), P::template dims<2>(n, nsp, p.red_smem)); return true;
+        case 4: f(P::template kernel<4>(), P::template dims<4>(n, nsp, p.red_smem)); return true;
+        case 8: f(P::template kernel<8>(), P::template dims<8>(n, nsp, p.red_smem)); return true;
+        case 16: f(P::template kernel<16>(), P::template dims<16>(n, nsp, p.red_smem)); return true;
+        default: return false;
     }
-    return false;
 }
 
-// Elements of global scratch per CTA for plan p (0: shared memory).
+// Elements of global scratch per CTA for plan p.
 template <class P>
 inline size_t pair_plan_scratch(const PairPlan& p, int n, int nsp)
 {
     size_t v = 0;
-    if (p.global) with_pair_instance<P>(p, n, nsp, [&](auto, const typename P::Dims& d) { v = (size_t)d.rec_doubles; });
+    with_pair_instance<P>(p, n, nsp, [&](auto, const typename P::Dims& d) { v = (size_t)d.rec_doubles; });
     return v;
 }
 
@@ -185,19 +179,19 @@ inline cudaError_t launch_persistent(Kernel fn, const Dims& d, const EvalArgs& a
 // first time it is used (a handful of instances per precision; setting it again is harmless).
 template <class P>
 inline cudaError_t launch_pair(const EvalArgs& a, int nsp, int num_sms, int smem_optin, cudaStream_t stream,
-                               const char** name, const char* shared_name, const char* global_name)
+                               const char** name, const char* kernel_name)
 {
     const PairPlan plan = pair_plan(a.n, nsp, a.batch, num_sms, P::kF32);
     cudaError_t err = cudaErrorInvalidValue;
     const bool found = with_pair_instance<P>(plan, a.n, nsp, [&](auto fn, const typename P::Dims& d) {
-        if (plan.global && (a.scratch == nullptr || (size_t)d.rec_doubles > a.scratch_stride)) return;
+        if (a.scratch == nullptr || (size_t)d.rec_doubles > a.scratch_stride) return;
         if (d.smem_bytes > (size_t)smem_optin) return;
         err = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
         if (err != cudaSuccess) return;
         const long long teams = (a.batch * nsp + d.C - 1) / d.C;
-        err = launch_persistent(fn, d, a, teams, plan.global ? eval_max_ctas(a.batch, num_sms) : 0, num_sms, stream);
+        err = launch_persistent(fn, d, a, teams, eval_max_ctas(a.batch, num_sms), num_sms, stream);
     });
-    *name = plan.global ? global_name : shared_name;
+    *name = kernel_name;
     return found ? err : cudaErrorInvalidValue;
 }
 
@@ -212,7 +206,7 @@ inline cudaError_t dispatch_eval(const EvalArgs& a, cudaStream_t stream, int num
         return launch_persistent(tc.fn, tc.d, a, (a.batch * nsp + tc.d.C - 1) / tc.d.C, 0, num_sms, stream);
     }
     if (!force_generic && a.n >= kPairMinN) {
-        return launch_pair<Prec64>(a, nsp, num_sms, smem_optin, stream, name, "eval_pair_kernel", "eval_pair_kernel(global)");
+        return launch_pair<Prec64>(a, nsp, num_sms, smem_optin, stream, name, "eval_pair_kernel");
     }
     const bool use_global = generic_needs_global(a.n, smem_optin);
     if (use_global && a.scratch == nullptr) return cudaErrorInvalidValue;
@@ -246,7 +240,7 @@ inline cudaError_t dispatch_eval_f32(const EvalArgs& a, cudaStream_t stream, int
         return launch_persistent(tc.fn, tc.d, a, (a.batch * nsp + tc.d.C - 1) / tc.d.C, 0, num_sms, stream);
     }
     if (a.n >= kPairMinN)
-        return launch_pair<Prec32>(a, nsp, num_sms, smem_optin, stream, name, "eval_pair_kernel<float>", "eval_pair_kernel<float>(global)");
+        return launch_pair<Prec32>(a, nsp, num_sms, smem_optin, stream, name, "eval_pair_kernel<float>");
     const size_t smem = generic_smem_bytes(a.n, nsp, sizeof(float));
     int per_sm = 1;
     cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, f32::eval_generic_kernel<kGenericThreads>,
