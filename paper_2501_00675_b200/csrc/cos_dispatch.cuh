@@ -70,16 +70,18 @@ constexpr int kPairMinN = 11, kPairThreads = 512;
 struct PairPlan {
     int C;           // instances per team
     bool red_smem;   // reduction arrays in shared memory instead of the scratch block
+    bool small;      // two CTAs of 256 threads per SM instead of one of 512
 };
 // The plan of one launch: how many instances a CTA takes at a time.
 inline PairPlan pair_plan(int n, int nsp, long long batch, int num_sms, bool f32)
 {
-    PairPlan p{2, false};
+    PairPlan p{2, false, false};
     if (!f32) {
-        if (n == 11) p.C = 16;
+        if (n == 11) p = (nsp == 1) ? PairPlan{8, false, true} : PairPlan{16, false, false};   // one species: two CTAs of 256
+                                           // threads with teams of 8: 0.203 ms against 0.216 (one CTA of 512, teams of 16)
         else if (n == 12) p.C = 8;
         else if (n == 13) p.C = 4;
-        else if (n == 14) p = (nsp == 1) ? PairPlan{1, true} : PairPlan{2, false};   // one instance: its reduction arrays
+        else if (n == 14) p = (nsp == 1) ? PairPlan{1, true, false} : PairPlan{2, false, false};   // one instance: its reduction arrays
                                                                     // (128 KB) fit in shared memory: 0.813 against 0.844 ms
         else p.C = (nsp == 1) ? 2 : 4;
     } else {                           // float records: half the L1/L2 traffic, larger teams pay off
@@ -87,7 +89,7 @@ inline PairPlan pair_plan(int n, int nsp, long long batch, int num_sms, bool f32
     }
     // shrink the team only when more than half of the SMs would get no team at all
     // (n = 16, batch 256: 128 teams of 2 on 148 SMs measured 1.58 ms against 1.74 ms for 256 teams of 1)
-    while (p.C > nsp && (batch * nsp + p.C - 1) / p.C < num_sms / 2) { p.C /= 2; p.red_smem = false; }
+    while (p.C > nsp && (batch * nsp + p.C - 1) / p.C < num_sms / 2) { p.C /= 2; p.red_smem = false; p.small = false; }
     return p;
 }
 
@@ -96,19 +98,26 @@ struct Prec64 {
     static constexpr bool kF32 = false;
     using Dims = f64::PairDims;
     template <int C> static auto kernel() { return f64::eval_pair_kernel<C, kPairThreads, 1, 8>; }
-    template <int C> static Dims dims(int n, int nsp, bool rs) { return f64::pair_dims<C>(n, kPairThreads, nsp, rs); }
+    template <int C> static auto kernel_small() { return f64::eval_pair_kernel<C, kPairThreads / 2, 2, 8>; }
+    template <int C> static Dims dims(int n, int nsp, bool rs, int threads = kPairThreads) { return f64::pair_dims<C>(n, threads, nsp, rs); }
 };
 struct Prec32 {
     static constexpr bool kF32 = true;
     using Dims = f32::PairDims;
     template <int C> static auto kernel() { return f32::eval_pair_kernel<C, kPairThreads, 1, 8>; }
-    template <int C> static Dims dims(int n, int nsp, bool rs) { return f32::pair_dims<C>(n, kPairThreads, nsp, rs); }
+    template <int C> static auto kernel_small() { return f32::eval_pair_kernel<C, kPairThreads / 2, 2, 8>; }
+    template <int C> static Dims dims(int n, int nsp, bool rs, int threads = kPairThreads) { return f32::pair_dims<C>(n, threads, nsp, rs); }
 };
 
 // Calls f(kernel, dims) for the kernel instance of plan p at order n (false: no such instance).
 template <class P, class F>
 inline bool with_pair_instance(const PairPlan& p, int n, int nsp, F&& f)
 {
+    if (p.small) {
+        if (p.C != 8) return false;
+        f(P::template kernel_small<8>(), P::template dims<8>(n, nsp, p.red_smem, kPairThreads / 2));
+        return true;
+    }
     switch (p.C) {
         case 1: f(P::template kernel<1>(), P::template dims<1>(n, nsp, p.red_smem)); return true;
         case 2: f(P::template kernel<2>(), P::template dims<2>(n, nsp, p.red_smem)); return true;
