@@ -50,8 +50,8 @@ struct TeamChoice32 { TeamKernel32 fn; f32::TeamDims d; };
 inline TeamChoice32 team_choice_f32(int n, int nsp)
 {
     if (n == 10) return {f32::eval_team_kernel<4, 160, 3>, f32::team_dims<4>(n, nsp)};
-    if (n == 9) return {f32::eval_team_kernel<8, 160, 3>, f32::team_dims<8>(n, nsp)};
-    if (n == 8) return {f32::eval_team_kernel<16, 160, 3>, f32::team_dims<16>(n, nsp)};
+    if (n == 9) return {f32::eval_team_kernel<8, 160, 4>, f32::team_dims<8>(n, nsp)};
+    if (n == 8) return {f32::eval_team_kernel<16, 160, 4>, f32::team_dims<16>(n, nsp)};
     return {f32::eval_team_kernel<32, 192, 2>, f32::team_dims<32>(n, nsp)};
 }
 
