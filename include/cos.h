@@ -11,7 +11,12 @@
  *   - plain C, no torch types.  Every pointer named d_* is a DEVICE pointer, every pointer named h_*
  *     is a HOST pointer; both are owned by the caller.  The library never frees, reallocates or keeps
  *     a caller pointer beyond the call, except the G0 table (borrowed until replaced/destroyed).
- *   - all floating point is IEEE FP64 (north_star; the paper itself ran FP32, reading R12).
+ *   - all floating point is IEEE FP64 (north_star; the paper itself ran FP32, reading R12), except inside the
+ *     *_f32 entry points, which say so.
+ *   - results are deterministic: the same call on the same inputs returns the same bits.  For n <= 10 the value of a
+ *     configuration does not depend on the batch it is part of; for n >= 11 the number of configurations a thread
+ *     block works on at a time follows the batch size, and with it the order of some sums: across different batch
+ *     sizes the values agree to rounding (about 1e-13 relative), not bit for bit.
  *   - calls on d_* buffers are ASYNCHRONOUS on the stream given to cos_create; results are valid
  *     after the caller synchronises that stream.  Calls on h_* buffers synchronise before returning.
  *   - return value: COS_OK (0) or a negative cos_status; cos_strerror() gives the text.  No
