@@ -373,3 +373,24 @@ def test_result_independent_of_batch_position_and_repeatable(torch_mod, ctx, n, 
         np.testing.assert_array_equal(c, a[:k])
     else:       # from order 11 the team size follows the batch (cos_dispatch.cuh: pair_plan), and with it the order in
         np.testing.assert_allclose(c, a[:k], rtol=1e-10)      # which the reduction sums its partial blocks
+
+
+@pytest.mark.parametrize("n,nsp", [(11, 1), (11, 2), (13, 1), (13, 2), (14, 1), (16, 1), (16, 2)])
+def test_sweep_shapes_sampled_outputs(torch_mod, ctx, oracle_mod, n, nsp):
+    """The team plans of orders 11..16 (cos_dispatch.cuh: pair_plan) at the batch sizes of the bench sweep -- two CTAs of
+    256 threads at n = 11, teams of 4 at n = 13, one instance with its reduction arrays in shared memory at n = 14,
+    teams of 2 / 4 at n = 16 -- checked against the oracle on a seeded sample that includes the first and the last
+    configuration."""
+    from harness import workloads as wl
+    B = wl.sweep_batch(n)
+    rng = np.random.default_rng(9000 + 10 * n + nsp)
+    Gup = rng.normal(size=(B, n, n)) / np.sqrt(n) + 0.5 * np.eye(n)
+    Gdn = rng.normal(size=(B, n, n)) / np.sqrt(n) + 0.5 * np.eye(n) if nsp == 2 else None
+    u = rng.uniform(0.5, 2.0, size=(B, n))
+    got = _gpu_eval(torch_mod, ctx, Gup, Gdn, 1.0, u, "connected")
+    assert np.all(np.isfinite(got))
+    idx = np.sort(rng.choice(B, size=64 if n <= 13 else 8, replace=False))
+    idx[0], idx[-1] = 0, B - 1
+    sub = lambda a: None if a is None else np.ascontiguousarray(a[idx])
+    st = check_parity(oracle_mod, got[idx], sub(Gup), sub(Gdn), 1.0, sub(u), "connected", label=f"sweep shape nsp={nsp}")
+    assert st["exceptions"] == 0, st
