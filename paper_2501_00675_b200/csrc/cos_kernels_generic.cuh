@@ -20,8 +20,7 @@ namespace cosb {
 
 // ------------------------------------------------------------------------------------------ a1
 // One thread per (b, i, j).  Table rows are L2 resident (1-8 MiB); two adjacent tau points per entry.
-// One entry G_s[b][i][j] (both species) of step a1; shared by build_G_kernel and the fused evaluation kernels so
-// that both produce bit-identical matrices.
+// One entry G_s[b][i][j] (both species) of step a1.
 // Off-diagonal value from the coordinates of the two vertices (reading R8: 2-point lerp on the tau grid,
 // antiperiodic branch for dtau <= 0, R9).
 __device__ __forceinline__ void g0_value(const BuildGArgs& a, int xi, int yi, int xj, int yj, double ti, double tj,
