@@ -92,7 +92,8 @@ def ncu_traffic(workload_name: str):
     try:
         with open(path) as f:
             rec = json.load(f).get(workload_name)
-        return None if rec is None else {"bytes": rec["dram_bytes"], "source": "profiles/r2_traffic.json: " + rec["capture"]}
+        return None if rec is None else {"bytes": rec["dram_bytes"], "source": "profiles/r2_traffic.json: " + rec["capture"],
+                                         "executed_over_algorithmic": rec.get("executed_over_algorithmic")}
     except (OSError, ValueError, KeyError):
         return None
 
@@ -423,6 +424,8 @@ def run_ours(args):
     if tr is not None:
         line["roofline"]["traffic"] = tr["bytes"]
         line["roofline"]["traffic_source"] = tr["source"]
+        # FP64 thread instructions executed (DFMA + DMUL + DADD, predicated on) / algorithmic FMAs, same ncu capture
+        line["roofline"]["fp64_executed_over_algorithmic"] = tr["executed_over_algorithmic"]
     if not args.no_cpu_baseline and world == 1:
         line["cpu_baseline"], sample = cpu_baseline(w)
         line["parity_sample"] = parity_on_sample(w, runner.out.cpu().numpy(), sample)
