@@ -97,15 +97,15 @@ inline PairPlan pair_plan(int n, int nsp, long long batch, int num_sms, bool f32
 struct Prec64 {
     static constexpr bool kF32 = false;
     using Dims = f64::PairDims;
-    template <int C> static auto kernel() { return f64::eval_pair_kernel<C, kPairThreads, 1, 8>; }
-    template <int C> static auto kernel_small() { return f64::eval_pair_kernel<C, kPairThreads / 2, 2, 8>; }
+    template <int C> static auto kernel() { return f64::eval_pair_kernel<C, kPairThreads, 1, 6>; }
+    template <int C> static auto kernel_small() { return f64::eval_pair_kernel<C, kPairThreads / 2, 2, 6>; }
     template <int C> static Dims dims(int n, int nsp, bool rs, int threads = kPairThreads) { return f64::pair_dims<C>(n, threads, nsp, rs); }
 };
 struct Prec32 {
     static constexpr bool kF32 = true;
     using Dims = f32::PairDims;
-    template <int C> static auto kernel() { return f32::eval_pair_kernel<C, kPairThreads, 1, 8>; }
-    template <int C> static auto kernel_small() { return f32::eval_pair_kernel<C, kPairThreads / 2, 2, 8>; }
+    template <int C> static auto kernel() { return f32::eval_pair_kernel<C, kPairThreads, 1, 6>; }
+    template <int C> static auto kernel_small() { return f32::eval_pair_kernel<C, kPairThreads / 2, 2, 6>; }
     template <int C> static Dims dims(int n, int nsp, bool rs, int threads = kPairThreads) { return f32::pair_dims<C>(n, threads, nsp, rs); }
 };
 
