@@ -58,8 +58,9 @@ inline TeamChoice32 team_choice_f32(int n, int nsp)
 // ---- pair kernel (orders 11..16): the team mapping with every item split over a lane pair ----
 // The records (Z, frontier, reduction arrays) live in a per-CTA block of global scratch served by L1/L2, so a CTA is
 // not limited by the 227 KB of an SM and works on a TEAM of several instances: every level then exposes that many
-// times more items per block barrier.  Measured (round 2, product build, kernel ms; "shared" = the round-1 kernel
-// with the records in shared memory, since removed):
+// times more items per block barrier.  Measured (round 2, product build, kernel ms, column windows of 8 -- the
+// windows of 6 adopted later take another 5-10 % off every figure; "shared" = the round-1 kernel with the records
+// in shared memory, since removed):
 //   one species  n=11: shared 0.221, C=8 0.226, C=16 0.216   n=12: shared 0.549, C=4 0.501, C=8 0.490, C=16 0.538
 //                n=13: shared 0.388, C=1 0.42, C=2 0.361, C=4 0.333, C=8 0.355   n=14: C=1 0.864, C=2 0.846, C=4 0.855
 //                n=15: C=1 1.214, C=2 1.107, C=4 1.126        n=16 (batch 256): C=1 1.740, C=2 1.577
