@@ -86,13 +86,13 @@ def get_workload(name: str, rank: int = 0):
 # ----------------------------------------------------------------------------------------------
 def ncu_traffic(workload_name: str):
     """dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel, per launch, parsed from the committed ncu
-    summary profiles/r2_traffic.json (written from one `ncu --set full` capture per workload; the file names the
+    summary profiles/r2_traffic.json.txt (written from one `ncu --set full` capture per workload; the file names the
     command).  None when the workload was not captured -- nothing is measured under a profiler in this run."""
-    path = os.path.join(ROOT, "profiles", "r2_traffic.json")
+    path = os.path.join(ROOT, "profiles", "r2_traffic.json.txt")
     try:
         with open(path) as f:
             rec = json.load(f).get(workload_name)
-        return None if rec is None else {"bytes": rec["dram_bytes"], "source": "profiles/r2_traffic.json: " + rec["capture"],
+        return None if rec is None else {"bytes": rec["dram_bytes"], "source": "profiles/r2_traffic.json.txt: " + rec["capture"],
                                          "executed_over_algorithmic": rec.get("executed_over_algorithmic")}
     except (OSError, ValueError, KeyError):
         return None
