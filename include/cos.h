@@ -15,8 +15,9 @@
  *     *_f32 entry points, which say so.
  *   - results are deterministic: the same call on the same inputs returns the same bits.  For n <= 10 the value of a
  *     configuration does not depend on the batch it is part of; for n >= 11 the number of configurations a thread
- *     block works on at a time follows the batch size, and with it the order of some sums: across different batch
- *     sizes the values agree to rounding (about 1e-13 relative), not bit for bit.
+ *     block works on at a time follows the batch size (and is smaller for the last, partial round of a batch), and with
+ *     it the order of some sums: across different batch sizes or positions in the batch the values agree to rounding
+ *     (about 1e-13 relative), not bit for bit.
  *   - calls on d_* buffers are ASYNCHRONOUS on the stream given to cos_create; results are valid
  *     after the caller synchronises that stream.  Calls on h_* buffers synchronise before returning.
  *   - return value: COS_OK (0) or a negative cos_status; cos_strerror() gives the text.  No

@@ -185,15 +185,14 @@ inline cudaError_t launch_persistent(Kernel fn, const Dims& d, const EvalArgs& a
     return cudaGetLastError();
 }
 
-// Launches the pair-kernel instance the plan names.  The opt-in shared-memory attribute of an instance is set the
-// first time it is used (a handful of instances per precision; setting it again is harmless).
+// Launches the pair-kernel instance plan p names, on the configurations [0, a.batch) of `a`.  The opt-in shared-memory
+// attribute of an instance is set when it is used (a handful of instances per precision; setting it again is harmless).
 template <class P>
-inline cudaError_t launch_pair(const EvalArgs& a, int nsp, int num_sms, int smem_optin, cudaStream_t stream,
-                               const char** name, const char* kernel_name)
+inline cudaError_t launch_pair_plan(const EvalArgs& a, const PairPlan& p, int nsp, int num_sms, int smem_optin,
+                                    cudaStream_t stream)
 {
-    const PairPlan plan = pair_plan(a.n, nsp, a.batch, num_sms, P::kF32);
     cudaError_t err = cudaErrorInvalidValue;
-    const bool found = with_pair_instance<P>(plan, a.n, nsp, [&](auto fn, const typename P::Dims& d) {
+    const bool found = with_pair_instance<P>(p, a.n, nsp, [&](auto fn, const typename P::Dims& d) {
         if (a.scratch == nullptr || (size_t)d.rec_doubles > a.scratch_stride) return;
         if (d.smem_bytes > (size_t)smem_optin) return;
         err = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
@@ -201,8 +200,51 @@ inline cudaError_t launch_pair(const EvalArgs& a, int nsp, int num_sms, int smem
         const long long teams = (a.batch * nsp + d.C - 1) / d.C;
         err = launch_persistent(fn, d, a, teams, eval_max_ctas(a.batch, num_sms), num_sms, stream);
     });
-    *name = kernel_name;
     return found ? err : cudaErrorInvalidValue;
+}
+
+// The tail of a batch.  A persistent grid works in rounds of one team per CTA; when the last round would occupy at most
+// half of the CTAs, its configurations are launched separately with the smallest team that still takes one round: a
+// round lasts about as long as its team is large (n = 12, batch 4096, teams of 8 on 148 CTAs: 3.46 rounds cost 4;
+// 3 rounds of 8 + 1 round of 4 cost 3.6).  Returns the number of configurations to run with plan p; *tail gets the
+// plan of the rest (tail->C == 0: no split).
+inline long long pair_tail_split(const PairPlan& p, int nsp, long long batch, int num_sms, PairPlan* tail)
+{
+    tail->C = 0; tail->red_smem = false; tail->small = false;
+    if (p.small || p.C / 2 < nsp) return batch;
+    const long long grid = num_sms;                                  // one CTA of 512 threads per SM
+    const long long teams = (batch * nsp + p.C - 1) / p.C;
+    const long long full = teams / grid, rem = teams - full * grid;
+    if (full < 1 || rem == 0 || rem > grid / 2) return batch;
+    const long long head = full * grid * p.C / nsp;                  // configurations of the full rounds
+    int c = p.C / 2;
+    while (c / 2 >= nsp && ((batch - head) * nsp + c / 2 - 1) / (c / 2) <= grid) c /= 2;
+    tail->C = c;
+    return head;
+}
+
+template <class P>
+inline cudaError_t launch_pair(const EvalArgs& a, int nsp, int num_sms, int smem_optin, cudaStream_t stream,
+                               const char** name, const char* kernel_name, int* launches)
+{
+    *name = kernel_name;
+    const PairPlan plan = pair_plan(a.n, nsp, a.batch, num_sms, P::kF32);
+    PairPlan tail;
+    const long long head = pair_tail_split(plan, nsp, a.batch, num_sms, &tail);
+    if (tail.C == 0) return launch_pair_plan<P>(a, plan, nsp, num_sms, smem_optin, stream);
+    EvalArgs h = a, t = a;
+    h.batch = head;
+    t.batch = a.batch - head;
+    const size_t es = P::kF32 ? sizeof(float) : sizeof(double);     // element size behind the input pointers
+    const size_t go = (size_t)head * a.n * a.n * es, uo = (size_t)head * a.n * es;
+    t.Gup = reinterpret_cast<const double*>(reinterpret_cast<const char*>(a.Gup) + go);
+    t.Gdn = reinterpret_cast<const double*>(reinterpret_cast<const char*>(a.Gdn) + go);
+    if (a.u) t.u = reinterpret_cast<const double*>(reinterpret_cast<const char*>(a.u) + uo);
+    t.out = a.out + head;
+    cudaError_t e = launch_pair_plan<P>(h, plan, nsp, num_sms, smem_optin, stream);
+    if (e != cudaSuccess) return e;
+    *launches = 2;
+    return launch_pair_plan<P>(t, tail, nsp, num_sms, smem_optin, stream);
 }
 
 inline cudaError_t dispatch_eval(const EvalArgs& a, cudaStream_t stream, int num_sms, int smem_optin,
@@ -216,7 +258,7 @@ inline cudaError_t dispatch_eval(const EvalArgs& a, cudaStream_t stream, int num
         return launch_persistent(tc.fn, tc.d, a, (a.batch * nsp + tc.d.C - 1) / tc.d.C, 0, num_sms, stream);
     }
     if (!force_generic && a.n >= kPairMinN) {
-        return launch_pair<Prec64>(a, nsp, num_sms, smem_optin, stream, name, "eval_pair_kernel");
+        return launch_pair<Prec64>(a, nsp, num_sms, smem_optin, stream, name, "eval_pair_kernel", launches);
     }
     const bool use_global = generic_needs_global(a.n, smem_optin);
     if (use_global && a.scratch == nullptr) return cudaErrorInvalidValue;
@@ -250,7 +292,7 @@ inline cudaError_t dispatch_eval_f32(const EvalArgs& a, cudaStream_t stream, int
         return launch_persistent(tc.fn, tc.d, a, (a.batch * nsp + tc.d.C - 1) / tc.d.C, 0, num_sms, stream);
     }
     if (a.n >= kPairMinN)
-        return launch_pair<Prec32>(a, nsp, num_sms, smem_optin, stream, name, "eval_pair_kernel<float>");
+        return launch_pair<Prec32>(a, nsp, num_sms, smem_optin, stream, name, "eval_pair_kernel<float>", launches);
     const size_t smem = generic_smem_bytes(a.n, nsp, sizeof(float));
     int per_sm = 1;
     cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, f32::eval_generic_kernel<kGenericThreads>,
