@@ -42,7 +42,8 @@ typedef enum cos_status {
     COS_EINVAL = -1,   /* bad argument: n out of range, batch < 0, NULL where not allowed, ntau < 2, ... */
     COS_ECUDA = -2,    /* CUDA runtime/driver error (no device, launch failure, ...) */
     COS_ENOMEM = -3,   /* device scratch allocation failed */
-    COS_ENOTABLE = -4  /* a call that needs the G0 table was made before cos_set_g0_table */
+    COS_ENOTABLE = -4, /* a call that needs the G0 table was made before cos_set_g0_table */
+    COS_ETOOBIG = -5   /* cos_eval_connected_noalloc: order or batch beyond the fixed capacity (COS_NOALLOC_*) */
 } cos_status;
 
 typedef struct cos_ctx cos_ctx; /* opaque; owns only internal device scratch */
@@ -171,6 +172,31 @@ int cos_set_loop_weight(cos_ctx* ctx, double n_f);
  * reduction over n_lines bits): correct for every size, not tuned. */
 int cos_eval_halfvertex(cos_ctx* ctx, int n_lines, long long batch, const double* d_W, const double* d_V,
                         int connected, double* d_out);
+
+/* Allocation-free evaluation of the connected sum, for callers that may not allocate device memory (code under CUDA
+ * graph capture, tight serving loops, harnesses that forbid cudaMalloc).  Same operation and argument meaning as
+ * cos_eval_connected (readings R1-R8), served by the pair
+ * kernel (orders >= 11, the kernel that keeps its records in global scratch) with BOTH its record space and its item
+ * descriptors in one file-scope `static __device__` array of COS_NOALLOC_SCRATCH_BYTES bytes that every GPU which
+ * loads the library holds until the process exits.  The call issues kernel launches only: no cudaMalloc, cudaFree or
+ * allocating library routine, and it does not touch the scratch the other entry points grow.
+ *   limits : COS_NOALLOC_MIN_ORDER <= n <= COS_NOALLOC_MAX_ORDER and 0 <= batch <= COS_NOALLOC_MAX_BATCH, else
+ *            COS_ETOOBIG (order or batch above the maximum) or COS_EINVAL (n below the minimum: those orders use no
+ *            scratch -- call cos_eval_connected; negative batch; NULL pointers).
+ *   team   : the largest team of instances per thread block, up to the one cos_eval_connected would take, whose
+ *            records for a full grid fit the array; values agree with cos_eval_connected to rounding (see the
+ *            determinism note above), bit for bit when the team is the same.
+ *   sharing: the array is shared by EVERY call on that GPU, from any ctx and any stream, and keeps the contents of the
+ *            last call.  Nothing in it has to start at zero (the descriptors are rewritten by every call, every record
+ *            is written before it is read).  Two calls that overlap on the GPU (different streams or contexts) race
+ *            on it and return garbage: serialise them.
+ * Asynchronous on the ctx stream like the other d_* calls. */
+#define COS_NOALLOC_MIN_ORDER 11
+#define COS_NOALLOC_MAX_ORDER 12
+#define COS_NOALLOC_MAX_BATCH (1LL << 20)
+#define COS_NOALLOC_SCRATCH_BYTES (32u << 20)
+int cos_eval_connected_noalloc(cos_ctx* ctx, int n, long long batch, const double* d_Gup, const double* d_Gdn,
+                               const double* d_u, double U, double* d_out);
 
 /* Cross-check switch: enable != 0 routes every later cos_eval_* call of this ctx, whatever the order, through the
  * plain one-thread-per-node kernel (the one orders 1..4 always use) instead of the tuned team / pair kernels; it

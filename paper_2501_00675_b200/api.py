@@ -18,7 +18,8 @@ import os
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libcos_b200.so")
 
-COS_OK, COS_EINVAL, COS_ECUDA, COS_ENOMEM, COS_ENOTABLE = 0, -1, -2, -3, -4
+COS_OK, COS_EINVAL, COS_ECUDA, COS_ENOMEM, COS_ENOTABLE, COS_ETOOBIG = 0, -1, -2, -3, -4, -5
+COS_NOALLOC_MIN_ORDER, COS_NOALLOC_MAX_ORDER, COS_NOALLOC_MAX_BATCH = 11, 12, 1 << 20
 COS_MAX_ORDER = 16
 
 _lib = None
@@ -36,6 +37,7 @@ SIGNATURES = {
     "cos_eval_all": (_int, [_vp, _int, _ll, _vp, _vp, _vp, _dbl, _vp]),
     "cos_eval_connected": (_int, [_vp, _int, _ll, _vp, _vp, _vp, _dbl, _vp]),
     "cos_eval_all_f32": (_int, [_vp, _int, _ll, _vp, _vp, _vp, _dbl, _vp]),
+    "cos_eval_connected_noalloc": (_int, [_vp, _int, _ll, _vp, _vp, _vp, _dbl, _vp]),
     "cos_eval_connected_f32": (_int, [_vp, _int, _ll, _vp, _vp, _vp, _dbl, _vp]),
     "cos_eval_connected_xt": (_int, [_vp, _int, _ll, _vp, _vp, _dbl, _vp, _dbl, _vp]),
     "cos_eval_connected_xt_host": (_int, [_vp, _int, _ll, _vp, _vp, _dbl, _vp, _dbl, _vp]),
@@ -217,6 +219,12 @@ class Context:
     def eval_connected(self, d_Gup, d_Gdn, d_out, U: float = 1.0, d_u=None):
         n, batch, gu, gd, u, out = self._eval_ptrs(d_Gup, d_Gdn, d_out, d_u)
         self._check(self._lib.cos_eval_connected(self._h, n, batch, gu, gd, u, float(U), out))
+
+    def eval_connected_noalloc(self, d_Gup, d_Gdn, d_out, U: float = 1.0, d_u=None):
+        """Allocation-free variant (include/cos.h: cos_eval_connected_noalloc): orders 11..12, scratch in a static
+        device array shared by every call on the GPU; CosError(COS_ETOOBIG) beyond the stated maximum."""
+        n, batch, gu, gd, u, out = self._eval_ptrs(d_Gup, d_Gdn, d_out, d_u)
+        self._check(self._lib.cos_eval_connected_noalloc(self._h, n, batch, gu, gd, u, float(U), out))
 
     def eval_all_f32(self, d_Gup, d_Gdn, d_out, U: float = 1.0, d_u=None):
         """FP32 variant (include/cos.h: cos_eval_all_f32); FP64 tensors in and out."""

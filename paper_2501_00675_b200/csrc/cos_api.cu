@@ -33,6 +33,7 @@ struct cos_ctx {
     unsigned char* team_tabs32[COS_MAX_ORDER + 1] = {};          // FP32 variant: table images of the team kernel
     float* g32 = nullptr;           size_t g32_bytes = 0;        // FP32 variant: converted copies of G_up, G_down, u
     void* mc = nullptr;             size_t mc_bytes = 0;         // cos_mc_run: proposal coordinates and weights
+    unsigned char* noalloc_scratch = nullptr;                    // device address of g_noalloc_scratch on this device
     cudaStream_t copy_stream = nullptr;                          // host path: H2D of chunk k+1 behind the kernels of chunk k
     cudaEvent_t copy_done[2] = {nullptr, nullptr};
     // bookkeeping
@@ -46,6 +47,12 @@ struct cos_ctx {
     std::vector<cudaEvent_t> ev;    // pairs (start, stop)
     size_t ev_used = 0;
 };
+
+// Scratch of cos_eval_connected_noalloc (include/cos.h): item descriptors of the order, then the record blocks of the
+// thread blocks.  One copy per GPU that loads the library, held until the process exits, shared by every call.  In host
+// code this name is a host-side stand-in, never a device address: cos_create asks the runtime for the address on its
+// device (cudaGetSymbolAddress) and the entry point passes that pointer to the kernels.
+static __device__ __align__(256) unsigned char g_noalloc_scratch[COS_NOALLOC_SCRATCH_BYTES];
 
 namespace {
 
@@ -302,6 +309,7 @@ const char* cos_strerror(int code)
         case COS_ECUDA: return "CUDA error (see cos_last_cuda_error)";
         case COS_ENOMEM: return "device scratch allocation failed";
         case COS_ENOTABLE: return "G0 table not set (call cos_set_g0_table first)";
+        case COS_ETOOBIG: return "order or batch beyond the fixed capacity of cos_eval_connected_noalloc (COS_NOALLOC_MAX_ORDER, COS_NOALLOC_MAX_BATCH)";
         default: return "unknown status";
     }
 }
@@ -343,6 +351,11 @@ int cos_create(cos_ctx** out, int device, void* cuda_stream)
     init_off_table_kernel<<<1, 1024, 0, c->stream>>>(c->off, count_off + 1);
     cudaError_t e = configure_kernels(c->smem_optin);
     if (e == cudaSuccess) e = cudaGetLastError();
+    if (e == cudaSuccess) {   // address of the static scratch on THIS device (the device set above is current)
+        void* p = nullptr;
+        e = cudaGetSymbolAddress(&p, g_noalloc_scratch);
+        c->noalloc_scratch = static_cast<unsigned char*>(p);
+    }
     if (e != cudaSuccess) {
         cudaFree(c->off);
         delete c;
@@ -415,6 +428,65 @@ int cos_eval_connected(cos_ctx* c, int n, long long batch, const double* d_Gup, 
     cudaSetDevice(c->device);
     c->last_launches = 0;
     return do_eval(c, n, batch, d_Gup, d_Gdn, d_u, U, d_out, 1);
+}
+
+int cos_eval_connected_noalloc(cos_ctx* c, int n, long long batch, const double* d_Gup, const double* d_Gdn,
+                               const double* d_u, double U, double* d_out)
+{
+    int rc = check_eval_args(c, n, batch, d_Gup, d_Gdn, d_out);
+    if (rc != COS_OK) return rc;
+    if (n > COS_NOALLOC_MAX_ORDER || batch > COS_NOALLOC_MAX_BATCH) return COS_ETOOBIG;
+    if (n < COS_NOALLOC_MIN_ORDER) return COS_EINVAL;
+    if (!c->noalloc_scratch) return COS_ECUDA;
+    c->last_launches = 0;
+    if (batch == 0) return COS_OK;
+    COS_CUDA(c, cudaSetDevice(c->device));
+    const int nsp = (d_Gdn == d_Gup) ? 1 : 2;
+    // layout of the array: [item descriptors of order n, rounded up to 256 B][record blocks, one per thread block]
+    const size_t dsc_bytes = (((size_t)1 << (n - f64::kPairB)) * f64::kPairDscWords * sizeof(uint32_t) + 255) & ~(size_t)255;
+    const size_t cap_doubles = ((size_t)COS_NOALLOC_SCRATCH_BYTES - dsc_bytes) / sizeof(double);
+    // the largest team, from the one cos_eval_connected would take downwards, whose records for a full grid fit
+    PairPlan p = pair_plan(n, nsp, batch, c->num_sms, false);
+    size_t per_cta = 0;
+    long long grid_cap = 0;
+    for (;;) {
+        per_cta = pair_plan_scratch<Prec64>(p, n, nsp);
+        if (per_cta == 0) return COS_EINVAL;
+        const long long teams = (batch * nsp + p.C - 1) / p.C;
+        long long grid = (long long)c->num_sms * (p.small ? 2 : 1);
+        if (grid > teams) grid = teams;
+        grid_cap = grid;
+        if (per_cta * (size_t)grid <= cap_doubles) break;
+        if (p.C / 2 >= nsp) { p = PairPlan{p.C / 2, false, false}; continue; }
+        grid_cap = (long long)(cap_doubles / per_cta);      // smallest team: fewer thread blocks than SMs
+        if (grid_cap < 1) return COS_ETOOBIG;
+        break;
+    }
+    uint32_t* dsc = reinterpret_cast<uint32_t*>(c->noalloc_scratch);
+    f64::pair_tables_kernel<<<32, 256, 0, c->stream>>>(n, dsc);
+    COS_CUDA(c, cudaGetLastError());
+    EvalArgs a{};
+    a.n = n; a.batch = batch; a.Gup = d_Gup; a.Gdn = d_Gdn; a.u = d_u; a.U = U; a.out = d_out;
+    a.connected = 1; a.off = c->off; a.loopf = -c->loop_weight;
+    a.tabs = c->noalloc_scratch;
+    a.scratch = reinterpret_cast<double*>(c->noalloc_scratch + dsc_bytes);
+    a.scratch_stride = per_cta;
+    cudaError_t err = cudaErrorInvalidValue;
+    const int smem_optin = c->smem_optin, num_sms = c->num_sms;
+    cudaStream_t stream = c->stream;
+    const bool t = timer_begin(c);
+    const bool found = with_pair_instance<Prec64>(p, n, nsp, [&](auto fn, const Prec64::Dims& d) {
+        if (d.smem_bytes > (size_t)smem_optin) return;
+        err = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
+        if (err != cudaSuccess) return;
+        err = launch_persistent(fn, d, a, (a.batch * nsp + d.C - 1) / d.C, grid_cap, num_sms, stream);
+    });
+    if (t) timer_end(c);
+    if (!found) return COS_EINVAL;
+    if (err != cudaSuccess) return fail_cuda(c, err);
+    c->last_launches = 2;
+    c->last_kernel = "eval_pair_kernel (static scratch)";
+    return COS_OK;
 }
 
 int cos_eval_all_f32(cos_ctx* c, int n, long long batch, const double* d_Gup, const double* d_Gdn,
