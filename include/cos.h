@@ -60,7 +60,8 @@ int cos_destroy(cos_ctx* ctx);
  *   spin: 0 = up, 1 = down, -1 = both species share this table.
  *   d_table: DEVICE, FP64, layout [Lx][Ly][ntau] with tau fastest; entry k holds G0 at
  *            tau_k = k*beta/(ntau-1), k = 0..ntau-1 (end points are 0+ and beta-; reading R8).
- *   The pointer is BORROWED until replaced or the ctx is destroyed.  Lx, Ly >= 1, ntau >= 2, beta > 0.
+ *   The pointer is BORROWED until replaced or the ctx is destroyed.  Lx, Ly >= 1, ntau >= 2, beta > 0,
+ *   Lx * Ly * ntau < 2^31 (COS_EINVAL otherwise).
  * (BASELINE.json north_star: "tabulated free propagator G0(x,tau)"; the paper takes G_ab as given.) */
 int cos_set_g0_table(cos_ctx* ctx, int spin, const double* d_table, int Lx, int Ly, int ntau, double beta);
 

@@ -285,11 +285,16 @@ int do_build_G(cos_ctx* c, int n, long long batch, const int* xy, const double* 
     a.Tup = c->table[0]; a.Tdn = c->table[1];
     a.Lx = c->Lx; a.Ly = c->Ly; a.ntau = c->ntau; a.beta = c->beta; a.g_diag = g_diag;
     a.Gup = gup; a.Gdn = (gdn == gup) ? nullptr : gdn;
-    const int per_cta = 256 / (n * n) > 0 ? 256 / (n * n) : 1;     // configurations per CTA pass (see the kernel)
-    long long blocks = (batch + per_cta - 1) / per_cta;
-    const long long cap = (long long)c->num_sms * 64;
+    a.rbeta = 1.0 / c->beta;                                        // IEEE division: the correctly rounded reciprocal
+    {
+        unsigned long long bits;
+        memcpy(&bits, &c->beta, sizeof bits);
+        a.fast_div = (bits & 0xFFFFFFFFFFFFFull) != 0xFFFFFFFFFFFFFull;
+    }
+    long long blocks = (batch + kBuildGCfgs - 1) / kBuildGCfgs;     // configurations per CTA pass (see the kernel)
+    const long long cap = (long long)c->num_sms * 8;
     if (blocks > cap) blocks = cap;
-    build_G_kernel<<<(unsigned)blocks, 256, 0, c->stream>>>(a);
+    build_G_kernel<<<(unsigned)blocks, build_G_threads(n), 0, c->stream>>>(a);
     COS_CUDA(c, cudaGetLastError());
     c->last_launches += 1;
     return COS_OK;
@@ -388,6 +393,7 @@ int cos_destroy(cos_ctx* c)
 int cos_set_g0_table(cos_ctx* c, int spin, const double* d_table, int Lx, int Ly, int ntau, double beta)
 {
     if (!c || !d_table || spin < -1 || spin > 1 || Lx < 1 || Ly < 1 || ntau < 2 || !(beta > 0.0)) return COS_EINVAL;
+    if ((long long)Lx * Ly * ntau >= (1LL << 31)) return COS_EINVAL;      // table entries are indexed with 32 bits
     const bool other_set = (spin >= 0) && c->table[1 - spin] != nullptr;
     if (other_set && (Lx != c->Lx || Ly != c->Ly || ntau != c->ntau || beta != c->beta)) return COS_EINVAL;
     if (spin == -1) c->table[0] = c->table[1] = d_table;

@@ -19,6 +19,8 @@ struct BuildGArgs {
     const double* Tdn;    // == Tup when shared
     int Lx, Ly, ntau;
     double beta;
+    double rbeta;         // RN(1 / beta), taken on the host
+    int fast_div;         // 1: x / beta by the FMA sequence of div_by_beta (0: the significand of beta is all ones)
     double g_diag;
     double* Gup;          // [batch][n][n]
     double* Gdn;          // nullptr: write Gup only

@@ -19,24 +19,45 @@
 namespace cosb {
 
 // ------------------------------------------------------------------------------------------ a1
-// One thread per (b, i, j).  Table rows are L2 resident (1-8 MiB); two adjacent tau points per entry.
-// One entry G_s[b][i][j] (both species) of step a1.
+// One thread per entry (i, j) of a configuration; a CTA stages the vertices of kBuildGCfgs configurations in shared
+// memory (coalesced loads) and walks the batch grid-strided.  Table rows are L2 resident (1-8 MiB); two adjacent
+// tau points per entry.
+
+// x / beta, correctly rounded, with the reciprocal y = RN(1 / beta) taken once on the host (Markstein's sequence for a
+// loop-invariant divisor: two FMA refinements, the residuals are exact and the last FMA rounds the quotient like a
+// division does).  The result is bit-identical to __ddiv_rn(x, beta); outside the range where the residuals cannot
+// underflow or overflow -- and when the host found the all-ones significand the theorem excludes -- the division
+// itself is used.  The kernel spent half of its instructions in the generic division.
+__device__ __forceinline__ double div_by_beta(const BuildGArgs& a, double x)
+{
+    if (!a.fast_div || !(x > 1e-200 && x < 1e200)) return __ddiv_rn(x, a.beta);
+    const double y = a.rbeta, b = a.beta;
+    double q = __dmul_rn(x, y);
+    double r = __fma_rn(-b, q, x);
+    q = __fma_rn(r, y, q);
+    r = __fma_rn(-b, q, x);
+    return __fma_rn(r, y, q);
+}
+
 // Off-diagonal value from the coordinates of the two vertices (reading R8: 2-point lerp on the tau grid,
 // antiperiodic branch for dtau <= 0, R9).
 __device__ __forceinline__ void g0_value(const BuildGArgs& a, int xi, int yi, int xj, int yj, double ti, double tj,
                                          double& gup, double& gdn)
 {
-    int dx = (xi - xj) % a.Lx; if (dx < 0) dx += a.Lx;
-    int dy = (yi - yj) % a.Ly; if (dy < 0) dy += a.Ly;
+    int dx = xi - xj, dy = yi - yj;
+    if ((unsigned)xi < (unsigned)a.Lx && (unsigned)xj < (unsigned)a.Lx) { if (dx < 0) dx += a.Lx; }   // sites in range: no division
+    else { dx %= a.Lx; if (dx < 0) dx += a.Lx; }
+    if ((unsigned)yi < (unsigned)a.Ly && (unsigned)yj < (unsigned)a.Ly) { if (dy < 0) dy += a.Ly; }
+    else { dy %= a.Ly; if (dy < 0) dy += a.Ly; }
     double dtau = ti - tj;
     double sign = 1.0;
     if (dtau <= 0.0) { dtau = __dadd_rn(dtau, a.beta); sign = -1.0; }     // R9: dtau == 0 is 0-
-    const double uu = __ddiv_rn(__dmul_rn(dtau, (double)(a.ntau - 1)), a.beta);
-    int k = (int)floor(uu);
+    const double uu = div_by_beta(a, __dmul_rn(dtau, (double)(a.ntau - 1)));
+    int k = (uu >= 2147483647.0) ? a.ntau - 2 : __double2int_rd(uu);      // floor; NaN and negatives clamp to 0 below
     k = min(k, a.ntau - 2);
     k = max(k, 0);
     const double f = __dsub_rn(uu, (double)k);
-    const size_t row = ((size_t)dx * a.Ly + dy) * (size_t)a.ntau + k;
+    const unsigned row = (unsigned)(dx * a.Ly + dy) * (unsigned)a.ntau + (unsigned)k;     // tables are < 2^32 entries (cos_set_g0_table)
     {
         const double t0 = __ldg(a.Tup + row), t1 = __ldg(a.Tup + row + 1);
         gup = sign * __fma_rn(f, __dsub_rn(t1, t0), t0);
@@ -49,27 +70,40 @@ __device__ __forceinline__ void g0_value(const BuildGArgs& a, int xi, int yi, in
     }
 }
 
-__device__ __forceinline__ void g0_entry(const BuildGArgs& a, long long b, int i, int j, double& gup, double& gdn)
-{
-    if (i == j) { gup = a.g_diag; gdn = a.g_diag; return; }
-    const int* pi = a.xy + (b * a.n + i) * 2;
-    const int* pj = a.xy + (b * a.n + j) * 2;
-    g0_value(a, pi[0], pi[1], pj[0], pj[1], a.tau[b * a.n + i], a.tau[b * a.n + j], gup, gdn);
-}
+constexpr int kBuildGThreads = 256;    // at most: the launch uses build_G_threads(n)
+constexpr int kBuildGCfgs = 8;         // configurations staged per CTA pass (measured at n = 10, batch 16384: 4: 25.5, 8: 23.1, 16: 24.9 us)
+// Threads per CTA: as many whole configurations as fit in 256 threads, one thread per entry, rounded up to a warp.
+__host__ __device__ inline int build_G_threads(int n) { return ((kBuildGThreads / (n * n)) * (n * n) + 31) & ~31; }
 
-// One thread per (b, i, j); a CTA walks whole configurations so that the index arithmetic stays 32-bit.
-__global__ void __launch_bounds__(256) build_G_kernel(BuildGArgs a)
+__global__ void __launch_bounds__(kBuildGThreads) build_G_kernel(BuildGArgs a)
 {
-    const int nn = a.n * a.n;
-    const int per_cta = 256 / nn > 0 ? 256 / nn : 1;          // configurations per CTA pass (n <= 16: nn <= 256)
-    const int local = threadIdx.x / nn, e = threadIdx.x - local * nn;
-    if (local >= per_cta) return;
-    const int i = e / a.n, j = e - i * a.n;
-    for (long long b = (long long)blockIdx.x * per_cta + local; b < a.batch; b += (long long)gridDim.x * per_cta) {
-        double gup, gdn;
-        g0_entry(a, b, i, j, gup, gdn);
-        a.Gup[b * nn + e] = gup;
-        if (a.Gdn) a.Gdn[b * nn + e] = gdn;
+    __shared__ int sx[kBuildGCfgs * kMaxN], sy[kBuildGCfgs * kMaxN];
+    __shared__ double st[kBuildGCfgs * kMaxN];
+    const int n = a.n, nn = n * n;
+    // a thread keeps its entry (i, j) for the whole launch and walks the configurations of a pass in steps of
+    // per_pass: every index inside the loop advances by a constant
+    const int per_pass = kBuildGThreads / nn;
+    const int cl = (int)threadIdx.x / nn, e = (int)threadIdx.x - cl * nn, i = e / n, j = e - i * n;
+    const bool live = cl < per_pass;
+    for (long long b0 = (long long)blockIdx.x * kBuildGCfgs; b0 < a.batch; b0 += (long long)gridDim.x * kBuildGCfgs) {
+        const int cfgs = (int)min((long long)kBuildGCfgs, a.batch - b0);
+        const int* xy = a.xy + b0 * n * 2;
+        const double* tau = a.tau + b0 * n;
+        __syncthreads();                                   // the previous pass has read its vertices
+        for (int v = threadIdx.x; v < cfgs * n; v += blockDim.x) {
+            sx[v] = xy[2 * v]; sy[v] = xy[2 * v + 1]; st[v] = tau[v];
+        }
+        __syncthreads();
+        if (!live) continue;
+        double* gu = a.Gup + b0 * nn + e;
+        double* gd = a.Gdn ? a.Gdn + b0 * nn + e : nullptr;
+        for (int c = cl; c < cfgs; c += per_pass) {        // consecutive threads: consecutive entries
+            const int vi = c * n + i, vj = c * n + j;
+            double gup = a.g_diag, gdn = a.g_diag;
+            if (i != j) g0_value(a, sx[vi], sy[vi], sx[vj], sy[vj], st[vi], st[vj], gup, gdn);
+            gu[c * nn] = gup;
+            if (gd) gd[c * nn] = gdn;
+        }
     }
 }
 

@@ -86,6 +86,36 @@ def test_build_G_two_tables_diag_and_ragged(torch_mod, ctx, oracle_mod):
         np.testing.assert_array_equal(Gdn.cpu().numpy(), ref_dn)
 
 
+@pytest.mark.parametrize("beta", [1.0 / 3.0, np.pi, 0.1, 7.0, 1e-3, 123.456, 0.125, 8.0, float(np.nextafter(2.0, 0.0)),
+                                  float(np.nextafter(1.0, 2.0)), 5e-324 * 2 ** 1000, 1.7e12])
+def test_build_G_division_by_beta_bit_exact(torch_mod, oracle_mod, beta):
+    """u = dtau (ntau - 1) / beta is taken with the reciprocal of beta and two FMA refinements (div_by_beta in
+    cos_kernels_generic.cuh); it must round like the division the oracle performs.  A quotient off by one ulp moves the
+    interpolation weight and with it the last bits of G, so every entry is compared bit for bit.  The values of beta
+    cover non-terminating binary fractions, powers of two, the all-ones significand (the generic division is used
+    there), the successor of 1, and magnitudes far from 1; times include equal pairs, pairs one ulp apart and the
+    ends of [0, beta); sites lie outside [0, L) as well (the modulo path)."""
+    torch = torch_mod
+    rng = np.random.default_rng(int(abs(np.log2(beta)) * 1000) % 100000)
+    L, ntau, B, n = 5, 257, 777, 8
+    T = rng.normal(size=(L, L, ntau))
+    xy = rng.integers(-2 * L, 3 * L, size=(B, n, 2)).astype(np.int32)
+    tau = rng.uniform(0, beta, size=(B, n))
+    tau[0, 1] = tau[0, 2]
+    tau[1, 3] = np.nextafter(tau[1, 4], 0.0)
+    tau[2, 0] = 0.0
+    tau[2, 5] = np.nextafter(beta, 0.0)
+    tau[3, :] = tau[3, 0] + np.arange(n) * (beta * 2.0 ** -40)        # clustered times (reading R15)
+    ref_up, _ = oracle_mod.build_G(xy, tau, T, None, beta, -0.5)
+    from paper_2501_00675_b200 import api
+    with api.Context() as c2:
+        c2.set_g0_table(_dev(torch, T), beta)
+        Gup = torch.empty((B, n, n), dtype=torch.float64, device="cuda")
+        c2.build_G(_dev(torch, xy), _dev(torch, tau), Gup, None, g_diag=-0.5)
+        torch.cuda.synchronize()
+        np.testing.assert_array_equal(Gup.cpu().numpy(), ref_up)
+
+
 # ------------------------------------------------------------------------------------------ a2..a5
 @pytest.mark.parametrize("n", list(range(1, 17)))
 def test_eval_every_order_dense(torch_mod, ctx, oracle_mod, n):
