@@ -44,11 +44,11 @@ __device__ __forceinline__ double div_by_beta(const BuildGArgs& a, double x)
 __device__ __forceinline__ void g0_value(const BuildGArgs& a, int xi, int yi, int xj, int yj, double ti, double tj,
                                          double& gup, double& gdn)
 {
+    // sites arrive reduced to [0, L) (build_G_kernel reduces them once per vertex when it stages them), so the
+    // difference needs one conditional add instead of a division
     int dx = xi - xj, dy = yi - yj;
-    if ((unsigned)xi < (unsigned)a.Lx && (unsigned)xj < (unsigned)a.Lx) { if (dx < 0) dx += a.Lx; }   // sites in range: no division
-    else { dx %= a.Lx; if (dx < 0) dx += a.Lx; }
-    if ((unsigned)yi < (unsigned)a.Ly && (unsigned)yj < (unsigned)a.Ly) { if (dy < 0) dy += a.Ly; }
-    else { dy %= a.Ly; if (dy < 0) dy += a.Ly; }
+    if (dx < 0) dx += a.Lx;
+    if (dy < 0) dy += a.Ly;
     double dtau = ti - tj;
     double sign = 1.0;
     if (dtau <= 0.0) { dtau = __dadd_rn(dtau, a.beta); sign = -1.0; }     // R9: dtau == 0 is 0-
@@ -91,7 +91,10 @@ __global__ void __launch_bounds__(kBuildGThreads) build_G_kernel(BuildGArgs a)
         const double* tau = a.tau + b0 * n;
         __syncthreads();                                   // the previous pass has read its vertices
         for (int v = threadIdx.x; v < cfgs * n; v += blockDim.x) {
-            sx[v] = xy[2 * v]; sy[v] = xy[2 * v + 1]; st[v] = tau[v];
+            int x = xy[2 * v], y = xy[2 * v + 1];
+            if ((unsigned)x >= (unsigned)a.Lx) { x %= a.Lx; if (x < 0) x += a.Lx; }      // (x_i - x_j) mod L from the residues
+            if ((unsigned)y >= (unsigned)a.Ly) { y %= a.Ly; if (y < 0) y += a.Ly; }
+            sx[v] = x; sy[v] = y; st[v] = tau[v];
         }
         __syncthreads();
         if (!live) continue;
