@@ -191,7 +191,8 @@ int cos_eval_halfvertex(cos_ctx* ctx, int n_lines, long long batch, const double
  *            last call.  Nothing in it has to start at zero (the descriptors are rewritten by every call, every record
  *            is written before it is read).  Two calls that overlap on the GPU (different streams or contexts) race
  *            on it and return garbage: serialise them.
- * Asynchronous on the ctx stream like the other d_* calls. */
+ * Asynchronous on the ctx stream like the other d_* calls.  Not covered by cos_enable_kernel_timer (the timer creates
+ * events on demand). */
 #define COS_NOALLOC_MIN_ORDER 11
 #define COS_NOALLOC_MAX_ORDER 12
 #define COS_NOALLOC_MAX_BATCH (1LL << 20)

@@ -480,14 +480,13 @@ int cos_eval_connected_noalloc(cos_ctx* c, int n, long long batch, const double*
     cudaError_t err = cudaErrorInvalidValue;
     const int smem_optin = c->smem_optin, num_sms = c->num_sms;
     cudaStream_t stream = c->stream;
-    const bool t = timer_begin(c);
+    // (not bracketed by the optional kernel timer: that would create events)
     const bool found = with_pair_instance<Prec64>(p, n, nsp, [&](auto fn, const Prec64::Dims& d) {
         if (d.smem_bytes > (size_t)smem_optin) return;
         err = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
         if (err != cudaSuccess) return;
         err = launch_persistent(fn, d, a, (a.batch * nsp + d.C - 1) / d.C, grid_cap, num_sms, stream);
     });
-    if (t) timer_end(c);
     if (!found) return COS_EINVAL;
     if (err != cudaSuccess) return fail_cuda(c, err);
     c->last_launches = 2;
