@@ -86,6 +86,33 @@ def test_build_G_two_tables_diag_and_ragged(torch_mod, ctx, oracle_mod):
         np.testing.assert_array_equal(Gdn.cpu().numpy(), ref_dn)
 
 
+@pytest.mark.parametrize("n", [1, 2, 3, 6, 7, 9, 11, 13, 14, 15, 16])
+def test_build_G_every_thread_shape(torch_mod, oracle_mod, n):
+    """build_G_kernel keeps one entry (i, j) per thread and as many whole configurations per pass as fit in 256 threads
+    (256, 64, 28, 7, 5, 3, 2, 1, 1, 1, 1 for these orders): every shape, with a batch that leaves a ragged last pass and
+    makes the grid loop more than once, bit for bit against the oracle, both tables."""
+    torch = torch_mod
+    rng = np.random.default_rng(600 + n)
+    L, ntau, beta = 6, 65, 2.5
+    B = 148 * 8 * 8 + 8 * 3 + 5                     # more than one pass of the capped grid, then a ragged tail
+    if n >= 13:
+        B = 148 * 8 * 8 // 4 + 13
+    Tu, Td = rng.normal(size=(L, L, ntau)), rng.normal(size=(L, L, ntau))
+    xy = rng.integers(0, L, size=(B, n, 2)).astype(np.int32)
+    tau = rng.uniform(0, beta, size=(B, n))
+    ref_up, ref_dn = oracle_mod.build_G(xy, tau, Tu, Td, beta, 0.75)
+    from paper_2501_00675_b200 import api
+    with api.Context() as c2:
+        c2.set_g0_table(_dev(torch, Tu), beta, spin=0)
+        c2.set_g0_table(_dev(torch, Td), beta, spin=1)
+        Gup = torch.full((B, n, n), float("nan"), dtype=torch.float64, device="cuda")
+        Gdn = torch.full((B, n, n), float("nan"), dtype=torch.float64, device="cuda")
+        c2.build_G(_dev(torch, xy), _dev(torch, tau), Gup, Gdn, g_diag=0.75)
+        torch.cuda.synchronize()
+        np.testing.assert_array_equal(Gup.cpu().numpy(), ref_up)
+        np.testing.assert_array_equal(Gdn.cpu().numpy(), ref_dn)
+
+
 @pytest.mark.parametrize("beta", [1.0 / 3.0, np.pi, 0.1, 7.0, 1e-3, 123.456, 0.125, 8.0, float(np.nextafter(2.0, 0.0)),
                                   float(np.nextafter(1.0, 2.0)), 5e-324 * 2 ** 1000, 1.7e12])
 def test_build_G_division_by_beta_bit_exact(torch_mod, oracle_mod, beta):
